@@ -1,0 +1,109 @@
+"""ORACLE-side comparators (test infrastructure): the comparison protocol of SURVEY.md §8(c-3)
+/ BASELINE.json north_star, applied to result arrays produced by ANY implementation.
+
+  spatial : sure(q) ⊆ G(q) ⊆ sure(q) ∪ band(q); rows duplicate-free; counts consistent.
+  kNN     : rules (1)..(5) of §8(c-3).
+Nothing here touches the CUDA path; inputs are plain numpy arrays.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import EPS, knn_distance_pairs
+
+
+def _keys(offsets: np.ndarray, indices: np.ndarray, n: int) -> np.ndarray:
+    offsets = np.asarray(offsets, dtype=np.int64)
+    rows = np.repeat(np.arange(offsets.shape[0] - 1, dtype=np.int64), np.diff(offsets))
+    return rows * np.int64(max(n, 1)) + np.asarray(indices, dtype=np.int64)
+
+
+def check_csr_format(offsets, indices, n: int, nq: int) -> None:
+    """Pin P4: offsets[0]=0, non-decreasing, offsets[nq]=total, indices in [0,n)."""
+    offsets = np.asarray(offsets)
+    assert offsets.shape[0] == nq + 1, "offsets must have nq+1 entries"
+    assert int(offsets[0]) == 0, "offsets[0] != 0"
+    assert np.all(np.diff(offsets.astype(np.int64)) >= 0), "offsets decrease"
+    total = int(offsets[-1])
+    assert total == len(indices), f"offsets[nq]={total} != len(indices)={len(indices)}"
+    if total:
+        ind = np.asarray(indices)
+        assert ind.min() >= 0 and ind.max() < n, "index out of range"
+
+
+def compare_spatial(n: int, orc, got, what: str = "") -> dict:
+    """orc = (offsets, indices, band) from oracle.spatial; got = (offsets, indices)."""
+    o_off, o_idx, o_band = orc
+    g_off, g_idx = got
+    nq = len(o_off) - 1
+    check_csr_format(g_off, g_idx, n, nq)
+    ko = _keys(o_off, o_idx, n)
+    kg = np.sort(_keys(g_off, g_idx, n))
+    assert np.all(np.diff(kg) > 0), f"{what}: duplicate index inside a row"
+    sure = ko[np.asarray(o_band) == 0]
+    missing = ~np.isin(sure, kg, assume_unique=True)
+    assert not missing.any(), (
+        f"{what}: {int(missing.sum())} sure pairs missing, first (q,i)="
+        f"{divmod(int(sure[missing][0]), max(n, 1))}")
+    extra = ~np.isin(kg, ko, assume_unique=True)
+    assert not extra.any(), (
+        f"{what}: {int(extra.sum())} pairs reported that are neither sure nor band, first (q,i)="
+        f"{divmod(int(kg[extra][0]), max(n, 1))}")
+    return dict(pairs=int(len(kg)), sure=int(len(sure)), band=int(len(ko) - len(sure)))
+
+
+def compare_counts(orc, counts, what: str = "") -> None:
+    """|sure| <= counts[q] <= |sure|+|band| per query (bit-exact where the band is empty)."""
+    o_off, _, o_band = orc
+    o_off = np.asarray(o_off, dtype=np.int64)
+    allc = np.diff(o_off)
+    bandc = np.add.reduceat(np.concatenate([np.asarray(o_band, dtype=np.int64), [0]]),
+                            np.minimum(o_off[:-1], len(o_band)))
+    bandc = np.where(allc == 0, 0, bandc)
+    counts = np.asarray(counts, dtype=np.int64)
+    bad = (counts < allc - bandc) | (counts > allc)
+    assert not bad.any(), f"{what}: {int(bad.sum())} counts outside [sure, sure+band], first q={int(np.argmax(bad))}"
+
+
+def compare_knn(prims, pkind: int, qpoints, k: int, orc, got, eps: float = EPS, what: str = "",
+                abs_tol: float = 0.0) -> None:
+    """orc = (idx[nq,k], dist64[nq,k]); got = (idx[nq,k] int32, dist[nq,k] fp32 or None).
+    abs_tol: absolute slack added to every distance tolerance (sphere primitives only, where
+    ||y-c|| - R cancels)."""
+    o_idx, o_d = orc
+    g_idx, g_d = got
+    g_idx = np.asarray(g_idx)
+    nq = o_idx.shape[0]
+    n = prims.shape[0]
+    kk = min(k, n)
+    assert g_idx.shape == (nq, k)
+    # (1) min(k,n) valid entries, padding only when n < k, no duplicates
+    assert np.all(g_idx[:, :kk] >= 0) and np.all(g_idx[:, :kk] < n), f"{what}: invalid index"
+    assert np.all(g_idx[:, kk:] == -1), f"{what}: padding must be -1"
+    if kk > 1:
+        s = np.sort(g_idx[:, :kk], axis=1)
+        assert np.all(np.diff(s, axis=1) > 0), f"{what}: duplicate neighbour in a row"
+    if kk == 0:
+        return
+    qids = np.repeat(np.arange(nq, dtype=np.int64), kk)
+    d_true = knn_distance_pairs(prims, pkind, qpoints, qids, g_idx[:, :kk].reshape(-1)).reshape(nq, kk)
+    Dk = o_d[:, kk - 1][:, None]
+    # (5b) every reported neighbour lies within D_k(1+eps)
+    assert np.all(d_true <= Dk * (1 + eps) + abs_tol), f"{what}: reported neighbour farther than D_k(1+eps)"
+    # (5a) every oracle neighbour strictly closer than D_k(1-eps) is reported
+    must = o_d[:, :kk] < Dk * (1 - eps) - abs_tol
+    key_g = np.sort((np.arange(nq, dtype=np.int64)[:, None] * n + g_idx[:, :kk]).reshape(-1))
+    key_o = (np.arange(nq, dtype=np.int64)[:, None] * n + o_idx[:, :kk])[must]
+    assert np.isin(key_o, key_g).all(), f"{what}: a neighbour strictly inside D_k is missing"
+    if g_d is not None:
+        g_d = np.asarray(g_d, dtype=np.float64)
+        assert np.all(np.isinf(g_d[:, kk:])), f"{what}: padding distance must be +inf"
+        gd = g_d[:, :kk]
+        # (2) ascending in fp32
+        assert np.all(np.diff(gd, axis=1) >= 0), f"{what}: distances not ascending"
+        # (3) position-wise agreement with the oracle distances
+        od = o_d[:, :kk]
+        assert np.all(np.abs(gd - od) <= eps * od + abs_tol), (
+            f"{what}: distance mismatch, max rel {np.max(np.abs(gd - od) / np.maximum(od, 1e-300)):.3e}")
+        # (4) the reported distance belongs to the reported index
+        assert np.all(np.abs(gd - d_true) <= eps * d_true + abs_tol), f"{what}: distance does not match its index"

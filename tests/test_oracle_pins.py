@@ -1,0 +1,269 @@
+"""Pins for the oracle (CPU only): the oracle is checked against what the mathematics fixes,
+never against itself alone.  SURVEY.md §8(c-5) P1..P12; BASELINE.json north_star."""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+from paper_2507_23700_b200 import datagen as dg
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "lattice_closed_forms.txt")
+
+
+def _golden():
+    interior, totals = {}, {}
+    for line in open(GOLD):
+        t = line.split()
+        if not t or t[0].startswith("#"):
+            continue
+        if t[0] == "total":
+            totals[(int(t[1]), int(t[2]))] = int(t[3])
+        else:
+            interior[(int(t[0]), int(t[1]))] = int(t[2])
+    return interior, totals
+
+
+def _modes(orc, prims, pkind, kind, r=None):
+    """None = brute force, plus two grids with different cell sizes."""
+    cell = orc.default_cell(prims, pkind, kind, r)
+    return [None, orc.Grid(prims, pkind, cell), orc.Grid(prims, pkind, 0.37 * cell)]
+
+
+@pytest.mark.parametrize("D,g", [(1, 10), (2, 6), (3, 5), (4, 4)])
+def test_lattice_radius_one_counts_and_total(orc, D, g):
+    # P2: count(x) = 1 + sum_a [(x_a>0) + (x_a<g-1)];  total = g^D + 2D g^(D-1) (g-1)
+    _, totals = _golden()
+    p = dg.lattice_points(g, D)
+    q = dg.sphere_queries(p, 1.0)
+    expect = 1 + (p > 0).sum(1) + (p < g - 1).sum(1)
+    for grid in _modes(orc, p, dg.POINT, "spatial", 1.0):
+        off, idx, band = orc.spatial(p, dg.POINT, q, dg.SPHERE, grid)
+        assert np.array_equal(np.diff(off), expect)
+        assert int(off[-1]) == totals[(D, g)]
+        # neighbours are exactly self and the axis neighbours (L2, closed, self included)
+        rows = np.repeat(np.arange(len(p)), np.diff(off))
+        d1 = np.abs(p[rows] - p[idx]).sum(1)
+        assert set(np.unique(d1)) <= {0.0, 1.0}
+        # pairs at exactly d = r are flagged as band, the self pair is not
+        assert np.array_equal(band == 1, d1 == 1.0)
+
+
+@pytest.mark.parametrize("D,r", [(1, 1), (1, 2), (2, 1), (2, 2), (3, 1), (3, 2), (3, 3), (4, 1), (4, 2)])
+def test_lattice_interior_counts(orc, D, r):
+    interior, _ = _golden()
+    g = 2 * r + 3
+    p = dg.lattice_points(g, D)
+    centre = np.full((1, D), r + 1, dtype=np.float32)
+    q = dg.sphere_queries(centre, float(r))
+    for grid in _modes(orc, p, dg.POINT, "spatial", float(r)):
+        off, idx, _ = orc.spatial(p, dg.POINT, q, dg.SPHERE, grid)
+        assert int(off[-1]) == interior[(D, r)]
+    # L-infinity or L1 norms would give (2r+1)^D or the cross-polytope count instead
+    if D == 3 and r == 2:
+        assert interior[(D, r)] not in (125, 25)
+
+
+@pytest.mark.parametrize("D", [1, 2, 3])
+def test_lattice_knn(orc, D):
+    # P2': k = 2D+1 at interior points -> self + 2D axis neighbours, distances (0,1,...,1)
+    g = 5
+    p = dg.lattice_points(g, D)
+    interior = np.all((p > 0) & (p < g - 1), axis=1)
+    qp = p[interior]
+    k = 2 * D + 1
+    for grid in _modes(orc, p, dg.POINT, "knn"):
+        idx, d = orc.knn(p, dg.POINT, qp, k, grid)
+        assert np.array_equal(idx[:, 0], np.nonzero(interior)[0])
+        assert np.all(d[:, 0] == 0.0) and np.all(d[:, 1:] == 1.0)
+        l1 = np.abs(p[idx] - qp[:, None, :]).sum(2)
+        assert np.all(l1[:, 1:] == 1.0)
+        # k = 1 with queries = points -> self at distance exactly 0
+        i1, d1 = orc.knn(p, dg.POINT, p, 1, grid)
+        assert np.array_equal(i1[:, 0], np.arange(len(p))) and np.all(d1 == 0.0)
+
+
+@pytest.mark.parametrize("D", [1, 2, 3])
+def test_box_lattice(orc, D):
+    # P3: unit cells as boxes; touching counts (closed sets)
+    g = 5
+    cells = dg.lattice_cells(g, D)
+    z = np.full(D, 2, dtype=np.float32)
+    q_cell = np.concatenate([z, z + 1])[None, :]
+    q_shrunk = np.concatenate([z + 0.25, z + 0.75])[None, :]
+    for grid in _modes(orc, cells, dg.BOX, "spatial"):
+        off, _, band = orc.spatial(cells, dg.BOX, q_cell, dg.BOX, grid)
+        assert int(off[-1]) == 3 ** D and not band.any()
+        off, idx, _ = orc.spatial(cells, dg.BOX, q_shrunk, dg.BOX, grid)
+        assert int(off[-1]) == 1
+        off, _, _ = orc.spatial(cells, dg.BOX, (z + 0.5)[None, :], dg.POINT, grid)
+        assert int(off[-1]) == 1
+        off, _, _ = orc.spatial(cells, dg.BOX, z[None, :], dg.POINT, grid)
+        assert int(off[-1]) == 2 ** D
+        # kNN to boxes: the containing cell is at distance 0, face neighbours at 0.5
+        qi, qd = orc.knn(cells, dg.BOX, (z + 0.5)[None, :], 1 + 2 * D, grid)
+        assert qd[0, 0] == 0.0 and np.all(qd[0, 1:] == 0.5)
+
+
+def test_one_dimensional_searchsorted(orc):
+    # P12: in 1-D a radius search is two binary searches on the sorted coordinates
+    rs = dg.rng(7)
+    x = np.sort(rs.random(5000).astype(np.float32))
+    s = rs.random(700).astype(np.float32)
+    r = np.float32(0.003)
+    q = dg.sphere_queries(s[:, None], r)
+    # closed ball in exact arithmetic on the fp32 inputs
+    lo = np.searchsorted(x.astype(np.float64), s.astype(np.float64) - np.float64(r), "left")
+    hi = np.searchsorted(x.astype(np.float64), s.astype(np.float64) + np.float64(r), "right")
+    for grid in _modes(orc, x[:, None], dg.POINT, "spatial", float(r)):
+        off, idx, band = orc.spatial(x[:, None], dg.POINT, q, dg.SPHERE, grid)
+        sure = np.diff(off) - np.add.reduceat(np.append(band, 0).astype(np.int64), np.minimum(off[:-1], len(band))) * (np.diff(off) > 0)
+        assert np.all(sure <= hi - lo) and np.all(hi - lo <= np.diff(off))
+        nb = band == 0
+        rows = np.repeat(np.arange(len(s)), np.diff(off))
+        assert np.all(idx[nb] >= lo[rows[nb]]) and np.all(idx[nb] < hi[rows[nb]])
+    # kNN in 1-D: the k nearest of a sorted array form a contiguous window
+    k = 5
+    i_b, d_b = orc.knn(x[:, None], dg.POINT, s[:, None], k)
+    ref = np.sort(np.abs(x[None, :].astype(np.float64) - s[:, None].astype(np.float64)), axis=1)[:, :k]
+    assert np.array_equal(d_b, ref)
+    srt = np.sort(i_b, axis=1)
+    assert np.all(srt[:, -1] - srt[:, 0] == k - 1)
+
+
+KINDS = [dg.POINT, dg.BOX, dg.SPHERE]
+
+
+def _rand_prims(kind, n, D, seed):
+    if kind == dg.POINT:
+        return dg.uniform_points(n, D, seed)
+    if kind == dg.BOX:
+        return dg.uniform_boxes(n, D, seed, 0.5 * n ** (-1.0 / D))
+    return dg.uniform_spheres(n, D, seed, 0.7 * n ** (-1.0 / D))
+
+
+def _naive_predicate(q, qkind, p, pkind, D):
+    """Independent, per-pair python restatement of SURVEY §8(c-1) used on tiny inputs only."""
+    q = q.astype(np.float64); p = p.astype(np.float64)
+
+    def pb(x, lo, hi):
+        return float((np.maximum(0, np.maximum(lo - x, x - hi)) ** 2).sum())
+    if qkind == dg.SPHERE:
+        s, r = q[:D], q[D]
+        if pkind == dg.POINT: return ((p - s) ** 2).sum(), r * r
+        if pkind == dg.BOX: return pb(s, p[:D], p[D:]), r * r
+        return ((p[:D] - s) ** 2).sum(), (r + p[D]) ** 2
+    if qkind == dg.BOX:
+        if pkind == dg.POINT: return float(not np.all((q[:D] <= p) & (p <= q[D:]))), 0.5
+        if pkind == dg.BOX: return float(not np.all((p[:D] <= q[D:]) & (q[:D] <= p[D:]))), 0.5
+        return pb(p[:D], q[:D], q[D:]), p[D] ** 2
+    if pkind == dg.POINT: return float(not np.all(p == q)), 0.5
+    if pkind == dg.BOX: return float(not np.all((p[:D] <= q) & (q <= p[D:]))), 0.5
+    return ((q - p[:D]) ** 2).sum(), p[D] ** 2
+
+
+@pytest.mark.parametrize("pkind,qkind", list(itertools.product(KINDS, KINDS)))
+def test_bruteforce_matches_naive_python(orc, pkind, qkind):
+    # P1 on tiny inputs: C++ brute force == per-pair python loop of the definition table
+    D, n, nq = 2, 60, 40
+    p = _rand_prims(pkind, n, D, 3)
+    q = _rand_prims(qkind, nq, D, 4)
+    if qkind == dg.SPHERE:
+        q[:, D] *= 2.0
+    if qkind == dg.POINT and pkind == dg.POINT:
+        q[:10] = p[:10]
+    off, idx, band = orc.spatial(p, pkind, q, qkind)
+    for j in range(nq):
+        got = set(idx[off[j]:off[j + 1]][band[off[j]:off[j + 1]] == 0].tolist())
+        exp = set()
+        for i in range(n):
+            t, T = _naive_predicate(q[j], qkind, p[i], pkind, D)
+            if t < T * (1 - 1e-6):
+                exp.add(i)
+        assert got == exp, (pkind, qkind, j)
+
+
+@pytest.mark.parametrize("D", [1, 2, 3, 5])
+@pytest.mark.parametrize("pkind", KINDS)
+def test_grid_equals_bruteforce(orc, D, pkind):
+    # P1/P11: Mode B must reproduce Mode A exactly (both fp64, same predicate)
+    n, nq = 1500, 300
+    p = _rand_prims(pkind, n, D, 10 + D)
+    for qkind in KINDS:
+        q = _rand_prims(qkind, nq, D, 20 + D)
+        if qkind == dg.SPHERE:
+            q[:, D] = np.float32(1.2 * n ** (-1.0 / D))
+        rr = float(q[0, D]) if qkind == dg.SPHERE else None
+        a = orc.spatial(p, pkind, q, qkind)
+        for grid in _modes(orc, p, pkind, "spatial", rr)[1:]:
+            b = orc.spatial(p, pkind, q, qkind, grid)
+            for x, y in zip(a, b):
+                assert np.array_equal(x, y), (D, pkind, qkind)
+    qp = dg.uniform_points(nq, D, 30 + D)
+    qp[::7] = qp[::7] * 3.0 - 1.0          # some queries far outside the scene
+    for k in (1, 4, 9):
+        ia, da = orc.knn(p, pkind, qp, k)
+        for grid in _modes(orc, p, pkind, "knn")[1:]:
+            ib, db = orc.knn(p, pkind, qp, k, grid)
+            assert np.array_equal(da, db) and np.array_equal(ia, ib), (D, pkind, k)
+
+
+def test_symmetry_and_monotonicity(orc):
+    # P5: i in row(j) <=> j in row(i) for a point self-search;  P7: r1<r2 => rows nested
+    p = dg.uniform_points(2000, 3, 5)
+    n = len(p)
+    r1, r2 = 0.05, 0.08
+    o1 = orc.spatial(p, dg.POINT, dg.sphere_queries(p, r1), dg.SPHERE)
+    o2 = orc.spatial(p, dg.POINT, dg.sphere_queries(p, r2), dg.SPHERE)
+    k1 = np.repeat(np.arange(n), np.diff(o1[0])) * n + o1[1]
+    kt = o1[1].astype(np.int64) * n + np.repeat(np.arange(n), np.diff(o1[0]))
+    assert np.array_equal(np.sort(k1), np.sort(kt))
+    k2 = np.repeat(np.arange(n), np.diff(o2[0])) * n + o2[1]
+    assert np.isin(k1, k2).all() and len(k2) > len(k1)
+    # huge r: every row is [0, n)
+    o3 = orc.spatial(p[:200], dg.POINT, dg.sphere_queries(p[:50], 10.0), dg.SPHERE)
+    assert np.array_equal(np.diff(o3[0]), np.full(50, 200))
+    # P8 (sanity): mean count ~ rho * V(r) * (1 - 1.125 r) in the unit cube
+    m = len(k1) / n
+    expect = 1 + n * 4 / 3 * np.pi * r1 ** 3 * (1 - 1.125 * r1)   # +1: the self pair
+    assert abs(m - expect) / expect < 0.1
+
+
+def test_knn_radius_consistency_and_edges(orc):
+    # P6: radius search at D_k(1+2eps) holds >= k hits incl. the kNN set; at D_k(1-2eps) < k
+    p = dg.uniform_points(3000, 3, 8)
+    qp = dg.uniform_points(100, 3, 9)
+    k = 7
+    idx, d = orc.knn(p, dg.POINT, qp, k)
+    assert np.all(np.diff(d, axis=1) >= 0)
+    for j in range(0, 100, 9):
+        q_hi = dg.sphere_queries(qp[j:j + 1], 1.0)
+        q_hi = q_hi.astype(np.float64)
+        off, ind, band = orc.spatial(p, dg.POINT, dg.sphere_queries(qp[j:j + 1], d[j, -1] * (1 + 1e-5)), dg.SPHERE)
+        assert set(idx[j].tolist()) <= set(ind.tolist())
+        off, ind, band = orc.spatial(p, dg.POINT, dg.sphere_queries(qp[j:j + 1], d[j, -1] * (1 - 1e-5)), dg.SPHERE)
+        assert len(ind) < k
+    # A8: n < k pads with -1 / +inf;  n = 0 gives empty rows
+    i2, d2 = orc.knn(p[:3], dg.POINT, qp[:5], 5)
+    assert np.all(i2[:, 3:] == -1) and np.all(np.isinf(d2[:, 3:])) and np.all(i2[:, :3] >= 0)
+    off, ind, _ = orc.spatial(p[:0], dg.POINT, dg.sphere_queries(qp[:5], 0.1), dg.SPHERE)
+    assert np.array_equal(off, np.zeros(6, dtype=np.int64)) and len(ind) == 0
+    # A21: negative radius matches nothing; r = 0 matches only coincident points (exact)
+    off, _, _ = orc.spatial(p, dg.POINT, dg.sphere_queries(p[:10], -1.0), dg.SPHERE)
+    assert int(off[-1]) == 0
+    off, ind, band = orc.spatial(p, dg.POINT, dg.sphere_queries(p[:10], 0.0), dg.SPHERE)
+    assert np.array_equal(ind, np.arange(10)) and not band.any()
+
+
+def test_sphere_primitive_knn_distance(orc):
+    # A4: distance to a sphere primitive is max(0, |y-c| - R); worked by hand
+    s = np.array([[0, 0, 0, 1.0], [10, 0, 0, 2.0]], dtype=np.float32)
+    y = np.array([[3, 4, 0], [0.5, 0, 0], [9, 0, 0]], dtype=np.float32)
+    idx, d = orc.knn(s, dg.SPHERE, y, 2)
+    assert np.allclose(d[0], [4.0, np.sqrt(49 + 16) - 2.0])
+    assert idx[1, 0] == 0 and d[1, 0] == 0.0
+    assert idx[2, 0] == 1 and d[2, 0] == 0.0 and np.isclose(d[2, 1], 8.0)
+    # box primitive: 0 inside, Euclidean to the nearest face/corner outside
+    b = np.array([[0, 0, 0, 1, 1, 1]], dtype=np.float32)
+    _, d = orc.knn(b, dg.BOX, np.array([[0.5, 0.5, 0.5], [2, 2, 1]], dtype=np.float32), 1)
+    assert d[0, 0] == 0.0 and np.isclose(d[1, 0], np.sqrt(2.0))
