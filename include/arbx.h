@@ -1,0 +1,145 @@
+/* arbx.h -- C ABI of the B200-native (sm_100a) linear-BVH build + batched search library.
+ *
+ * The operations are those of arXiv 2507.23700 ("The ArborX library: version 2.0"),
+ * cited below as PAPER.md:Lnn (line of /root/reference/PAPER.md) + section:
+ *   - an index is built over user primitives (§2.2 "BVH ... constructor");
+ *   - spatial queries return, per query, the primitives that satisfy it, as
+ *     `indices` + `offsets` (CSR) (§2.1.1; L112-115, §2.2 query overload 3);
+ *   - the same search with a pure callback stores nothing; our instance of it counts
+ *     (§2.2 query overload 1; L303 Table 1 "Query (count)");
+ *   - nearest queries return the k closest primitives, distance measured to the stored
+ *     geometry ("fine" search, §2.1.2);
+ *   - every call takes an execution space = CUDA stream.
+ *
+ * Conventions
+ *   Pointers marked DEVICE must be device memory accessible from the current CUDA device;
+ *   pointers marked HOST are ordinary host memory.  The caller owns every buffer it passes;
+ *   the library never returns device memory.  The handle owns the tree and a private copy
+ *   of the geometry ("behave like a container"): `prims` may be released once
+ *   the build has completed on `stream`.  Per-call scratch is taken from the CUDA
+ *   stream-ordered allocator on `stream` and released before the call returns (in stream
+ *   order); nothing per-query is stored in the handle, so several queries may run
+ *   concurrently on one handle from different streams.
+ *   Using a handle on another stream than the one it was built on requires the caller to
+ *   order that stream after the build (event or synchronize).
+ *
+ *   Layout (row-major fp32):   POINT : dim floats            (coordinates)
+ *                              BOX   : 2*dim floats          (lo[dim] then hi[dim])
+ *                              SPHERE: dim+1 floats          (centre[dim] then radius)
+ *   1 <= dim <= 10.   0 <= n <= 2^30.   0 <= nq <= 2^30.
+ *
+ *   All geometric tests are CLOSED (touching counts), Euclidean, no self-exclusion.
+ *   NaN/Inf coordinates and inverted boxes are not validated (results undefined).
+ *   A SPHERE query with negative radius matches nothing.
+ *
+ *   Errors: every entry point returns an arbx_status; nothing throws or aborts.
+ *   arbx_last_error() gives a thread-local human-readable detail for the last failure.
+ */
+#ifndef ARBX_H_
+#define ARBX_H_
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define ARBX_API __attribute__((visibility("default")))
+#else
+#define ARBX_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct arbx_index_s* arbx_handle;   /* opaque; owns the device tree */
+typedef void* arbx_stream;                  /* a cudaStream_t (NULL = legacy default stream) */
+
+typedef enum { ARBX_POINT = 0, ARBX_BOX = 1, ARBX_SPHERE = 2 } arbx_kind;
+
+typedef enum {
+  ARBX_OK = 0,
+  ARBX_ERR_INVALID_ARG = 1, /* null pointer with non-zero count, dim/kind/k out of range, n<0 */
+  ARBX_ERR_UNSUPPORTED = 2, /* n or nq > 2^30, k > ARBX_K_MAX                                 */
+  ARBX_ERR_CAPACITY = 3,    /* indices_capacity < total (offsets and *total_host are valid)   */
+  ARBX_ERR_OVERFLOW = 4,    /* total > INT32_MAX: int32 offsets cannot hold it                */
+  ARBX_ERR_CUDA = 5,        /* a CUDA runtime call failed (detail in arbx_last_error)         */
+  ARBX_ERR_OOM = 6          /* device allocation failed                                       */
+} arbx_status;
+
+#define ARBX_MAX_DIM 10
+#define ARBX_K_MAX 256      /* k <= 32 runs on the register heap, 32 < k <= 256 on a local-memory heap */
+
+/* Build the index (PAPER.md:L101-103 constructor; internals L293-295: space-filling codes,
+ * sort, bottom-up hierarchy with bounding volumes).  Asynchronous on `stream` except for
+ * allocation.  prims: DEVICE, n rows in the layout of `kind`.  n == 0 gives a valid empty
+ * handle (PAPER.md:L120 empty()).  *out is written only on ARBX_OK.                        */
+ARBX_API arbx_status arbx_build(const float* prims, int64_t n, int dim, arbx_kind kind,
+                       arbx_stream stream, arbx_handle* out);
+
+/* Release the handle's device memory in stream order on `stream`. NULL is accepted.        */
+ARBX_API arbx_status arbx_destroy(arbx_handle h, arbx_stream stream);
+
+/* PAPER.md:L119 size().  HOST out pointer; no synchronisation.                              */
+ARBX_API arbx_status arbx_size(arbx_handle h, int64_t* n);
+
+/* PAPER.md:L121 bounds(): bounding box of all primitives.  lo_host/hi_host: HOST, dim floats
+ * each.  Synchronises `stream`.  For an empty index lo=+inf, hi=-inf.                        */
+ARBX_API arbx_status arbx_bounds(arbx_handle h, float* lo_host, float* hi_host, arbx_stream stream);
+
+/* Count-only search = the pure-callback query whose callback increments a counter
+ * (PAPER.md:L104-106, L131, L303).  qkind SPHERE = radius search (centre, r) (PAPER.md:L69
+ * "a pair of a query point and a radius"); BOX = box intersection; POINT =
+ * primitives containing the point.  queries: DEVICE, nq rows in the layout
+ * of qkind with the handle's dim.  counts: DEVICE int32[nq], counts[q] = number of
+ * primitives matching query q (caller's query order).  Asynchronous on `stream`.            */
+ARBX_API arbx_status arbx_query_count(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                             int32_t* counts, arbx_stream stream);
+
+/* Storage search (PAPER.md:L69 v1 "indices and offsets"; L112-115 overload 3).
+ * offsets: DEVICE int32[nq+1]; offsets[0]=0, offsets[q+1]-offsets[q] = matches of query q,
+ * offsets[nq] = total.  indices: DEVICE int32[indices_capacity] or NULL; the slice
+ * [offsets[q], offsets[q+1]) holds the positions, in the caller's prims array, of the
+ * primitives matching query q, in unspecified order.  total_host: HOST int64, may be NULL.
+ * The call enqueues count + scan, synchronises `stream` ONCE to learn the total, then:
+ *   indices == NULL               -> returns ARBX_OK (offsets and *total_host valid);
+ *   total > INT32_MAX             -> ARBX_ERR_OVERFLOW (*total_host valid, offsets not);
+ *   indices_capacity < total      -> ARBX_ERR_CAPACITY (offsets and *total_host valid);
+ *   otherwise enqueues the fill pass and returns without a second synchronisation.          */
+ARBX_API arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                               int32_t* offsets, int32_t* indices, int64_t indices_capacity,
+                               int64_t* total_host, arbx_stream stream);
+
+/* k nearest primitives to each query point ("a pair of a query point and a
+ * number of neighbors"; L79 distance to the stored geometry: point ||x-y||, box point-box
+ * distance (0 inside), sphere max(0,||y-c||-R)).  qpoints: DEVICE nq*dim.  One k per call,
+ * 1 <= k <= ARBX_K_MAX.  indices: DEVICE int32[nq*k]; distances: DEVICE fp32[nq*k] or NULL.
+ * Row q holds min(k,n) neighbours by ascending Euclidean distance (not squared); ties in
+ * unspecified order; when n < k the row is padded with index -1 / distance +inf.
+ * Asynchronous on `stream`.                                                                 */
+ARBX_API arbx_status arbx_query_knn(arbx_handle h, const float* qpoints, int64_t nq, int k,
+                           int32_t* indices, float* distances, arbx_stream stream);
+
+/* Stable LSD radix sort of (key, value) pairs, exposed for tests of build step B3
+ * ("Sorting in both construction and search").  keys: DEVICE, sorted in place
+ * on bits [0, key_bits); values: DEVICE uint32[n] or NULL (then only keys are sorted).
+ * key_bytes is 4 or 8.  Asynchronous on `stream`.                                           */
+ARBX_API arbx_status arbx_sort_pairs(void* keys, uint32_t* values, int64_t n, int key_bytes, int key_bits,
+                            arbx_stream stream);
+
+/* Structural self-check of the tree (test hook for SURVEY.md §8(c-5) pin P9): verifies on
+ * the device that sorted codes are non-decreasing, the leaf permutation is a permutation,
+ * every node is reachable exactly once from the root, every stored child box equals the
+ * union of that child's contents bit for bit.  *violations_host (HOST) = number of failed
+ * checks (0 = valid).  Synchronises `stream`.                                               */
+ARBX_API arbx_status arbx_debug_validate(arbx_handle h, int64_t* violations_host, arbx_stream stream);
+
+/* Number of kernels this library has launched in the calling process (for bench.py's
+ * gpu_launches claim).                                                                      */
+ARBX_API int64_t arbx_launch_count(void);
+
+ARBX_API const char* arbx_status_string(arbx_status s);
+ARBX_API const char* arbx_last_error(void);          /* thread-local detail of the last failure */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARBX_H_ */

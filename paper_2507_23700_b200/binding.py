@@ -1,0 +1,235 @@
+"""Thin Python binding of the C ABI in include/arbx.h (argument marshalling only).
+
+Every step of the hot path runs inside libarbx.so (hand-written sm_100a kernels); PyTorch is
+used for device memory and streams.  There is NO CPU fallback: if the shared library is
+missing or no CUDA device is present, calls raise.
+
+The functions carry the ABI's names (arbx_build, arbx_query_count, arbx_query_spatial,
+arbx_query_knn, ...).  `Index` is a small convenience wrapper owning one handle.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+POINT, BOX, SPHERE = 0, 1, 2
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CAPACITY, ERR_OVERFLOW, ERR_CUDA, ERR_OOM = range(7)
+K_MAX = 256
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libarbx.so")
+
+EXPORTS = (
+    "arbx_build", "arbx_destroy", "arbx_size", "arbx_bounds", "arbx_query_count",
+    "arbx_query_spatial", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
+    "arbx_launch_count", "arbx_status_string", "arbx_last_error",
+)
+
+
+class ArbxError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        L = lib()
+        super().__init__(f"{where}: {L.arbx_status_string(status).decode()} -- {L.arbx_last_error().decode()}")
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libarbx.so (built by `make -C paper_2507_23700_b200/csrc` or __graft_entry__.build())."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} is missing: build it with `python -c 'import __graft_entry__ as g; g.build()'` "
+                "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+        L.arbx_build.argtypes = [vp, i64, i32, i32, vp, ctypes.POINTER(vp)]
+        L.arbx_destroy.argtypes = [vp, vp]
+        L.arbx_size.argtypes = [vp, ctypes.POINTER(i64)]
+        L.arbx_bounds.argtypes = [vp, vp, vp, vp]
+        L.arbx_query_count.argtypes = [vp, vp, i64, i32, vp, vp]
+        L.arbx_query_spatial.argtypes = [vp, vp, i64, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.arbx_query_knn.argtypes = [vp, vp, i64, i32, vp, vp, vp]
+        L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
+        L.arbx_debug_validate.argtypes = [vp, ctypes.POINTER(i64), vp]
+        L.arbx_launch_count.restype = i64
+        L.arbx_status_string.restype = ctypes.c_char_p
+        L.arbx_status_string.argtypes = [i32]
+        L.arbx_last_error.restype = ctypes.c_char_p
+        for name in EXPORTS[:9]:
+            getattr(L, name).restype = i32
+        _lib = L
+    return _lib
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dev_f32(t: torch.Tensor, what: str) -> torch.Tensor:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda):
+        raise TypeError(f"{what} must be a CUDA tensor (no CPU path exists)")
+    if t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError(f"{what} must be contiguous float32")
+    return t
+
+
+def _ptr(t) -> int:
+    return 0 if t is None or t.numel() == 0 else t.data_ptr()
+
+
+def row_width(kind: int, dim: int) -> int:
+    return dim if kind == POINT else 2 * dim if kind == BOX else dim + 1
+
+
+def _check(st: int, where: str):
+    if st != OK:
+        raise ArbxError(st, where)
+
+
+# ---- functions named after the ABI ----------------------------------------------------------
+def arbx_build(prims: torch.Tensor, dim: int, kind: int, stream=None) -> int:
+    prims = _dev_f32(prims, "prims")
+    n = prims.numel() // row_width(kind, dim) if prims.numel() else 0
+    h = ctypes.c_void_p()
+    _check(lib().arbx_build(_ptr(prims), n, dim, kind, _stream(stream), ctypes.byref(h)), "arbx_build")
+    return h.value
+
+
+def arbx_destroy(handle: int, stream=None) -> None:
+    _check(lib().arbx_destroy(handle, _stream(stream)), "arbx_destroy")
+
+
+def arbx_size(handle: int) -> int:
+    n = ctypes.c_int64()
+    _check(lib().arbx_size(handle, ctypes.byref(n)), "arbx_size")
+    return n.value
+
+
+def arbx_bounds(handle: int, dim: int, stream=None):
+    lo = (ctypes.c_float * dim)()
+    hi = (ctypes.c_float * dim)()
+    _check(lib().arbx_bounds(handle, ctypes.addressof(lo), ctypes.addressof(hi), _stream(stream)), "arbx_bounds")
+    return list(lo), list(hi)
+
+
+def arbx_query_count(handle: int, queries: torch.Tensor, nq: int, qkind: int, counts: torch.Tensor,
+                     stream=None) -> None:
+    _check(lib().arbx_query_count(handle, _ptr(queries), nq, qkind, _ptr(counts), _stream(stream)),
+           "arbx_query_count")
+
+
+def arbx_query_spatial(handle: int, queries: torch.Tensor, nq: int, qkind: int, offsets: torch.Tensor,
+                       indices, capacity: int, stream=None, raise_on_capacity: bool = True):
+    """Returns (status, total)."""
+    total = ctypes.c_int64()
+    st = lib().arbx_query_spatial(handle, _ptr(queries), nq, qkind, offsets.data_ptr(),
+                                  0 if indices is None else indices.data_ptr(), capacity,
+                                  ctypes.byref(total), _stream(stream))
+    if st != OK and (raise_on_capacity or st != ERR_CAPACITY):
+        raise ArbxError(st, "arbx_query_spatial")
+    return st, total.value
+
+
+def arbx_query_knn(handle: int, qpoints: torch.Tensor, nq: int, k: int, indices: torch.Tensor,
+                   distances, stream=None) -> None:
+    _check(lib().arbx_query_knn(handle, _ptr(qpoints), nq, k, _ptr(indices),
+                                0 if distances is None else _ptr(distances), _stream(stream)),
+           "arbx_query_knn")
+
+
+def arbx_sort_pairs(keys: torch.Tensor, values, key_bits: int, stream=None) -> None:
+    assert keys.is_cuda and keys.is_contiguous() and keys.element_size() in (4, 8)
+    _check(lib().arbx_sort_pairs(_ptr(keys), 0 if values is None else _ptr(values), keys.numel(),
+                                 keys.element_size(), key_bits, _stream(stream)), "arbx_sort_pairs")
+
+
+def arbx_debug_validate(handle: int, stream=None) -> int:
+    v = ctypes.c_int64()
+    _check(lib().arbx_debug_validate(handle, ctypes.byref(v), _stream(stream)), "arbx_debug_validate")
+    return v.value
+
+
+def arbx_launch_count() -> int:
+    return int(lib().arbx_launch_count())
+
+
+# ---- convenience wrapper -----------------------------------------------------------------------
+class Index:
+    """One BVH over `prims` (CUDA float32 [n, row_width]).  PAPER.md:L89-123 (BVH class)."""
+
+    def __init__(self, prims: torch.Tensor, kind: int = POINT, dim: int | None = None, stream=None):
+        prims = _dev_f32(prims, "prims")
+        if dim is None:
+            if prims.dim() != 2:
+                raise ValueError("give dim= for a flat prims array")
+            w = prims.shape[1]
+            dim = w if kind == POINT else w // 2 if kind == BOX else w - 1
+        self.dim, self.kind, self.device = dim, kind, prims.device
+        self.handle = arbx_build(prims, dim, kind, stream)
+
+    def close(self, stream=None):
+        if getattr(self, "handle", None):
+            arbx_destroy(self.handle, stream)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def size(self) -> int:
+        return arbx_size(self.handle)
+
+    def empty(self) -> bool:
+        return self.size() == 0
+
+    def bounds(self, stream=None):
+        return arbx_bounds(self.handle, self.dim, stream)
+
+    def _nq(self, queries: torch.Tensor, qkind: int) -> int:
+        _dev_f32(queries, "queries")
+        return queries.numel() // row_width(qkind, self.dim)
+
+    def query_count(self, queries: torch.Tensor, qkind: int = SPHERE, stream=None) -> torch.Tensor:
+        nq = self._nq(queries, qkind)
+        counts = torch.empty(nq, dtype=torch.int32, device=self.device)
+        arbx_query_count(self.handle, queries, nq, qkind, counts, stream)
+        return counts
+
+    def query_spatial(self, queries: torch.Tensor, qkind: int = SPHERE, capacity: int | None = None,
+                      stream=None):
+        """CSR result (offsets int32[nq+1], indices int32[total]).  With `capacity` (an upper
+        bound the caller knows) the whole query is one ABI call; otherwise a first call with
+        indices=NULL learns the total (count + scan) and a second call fills."""
+        nq = self._nq(queries, qkind)
+        offsets = torch.empty(nq + 1, dtype=torch.int32, device=self.device)
+        if capacity is not None:
+            indices = torch.empty(capacity, dtype=torch.int32, device=self.device)
+            st, total = arbx_query_spatial(self.handle, queries, nq, qkind, offsets, indices, capacity,
+                                           stream, raise_on_capacity=False)
+            if st == OK:
+                return offsets, indices[:total]
+        else:
+            _, total = arbx_query_spatial(self.handle, queries, nq, qkind, offsets, None, 0, stream)
+        indices = torch.empty(total, dtype=torch.int32, device=self.device)
+        arbx_query_spatial(self.handle, queries, nq, qkind, offsets, indices, total, stream)
+        return offsets, indices
+
+    def query_knn(self, qpoints: torch.Tensor, k: int, want_distances: bool = True, stream=None):
+        nq = self._nq(qpoints, POINT)
+        idx = torch.empty((nq, k), dtype=torch.int32, device=self.device)
+        dist = torch.empty((nq, k), dtype=torch.float32, device=self.device) if want_distances else None
+        arbx_query_knn(self.handle, qpoints, nq, k, idx, dist, stream)
+        return idx, dist
+
+    def validate(self, stream=None) -> int:
+        return arbx_debug_validate(self.handle, stream)

@@ -1,0 +1,265 @@
+// api.cu -- the C ABI of include/arbx.h: argument validation, handle ownership, scratch
+// management and the order of the hot-path steps:
+//   build   : B1 bounds -> B2 codes -> B3 sort -> B4 leaves -> B5+B6 hierarchy/refit
+//   count   : Q1 query codes -> Q2 sort -> T1 traversal (count)
+//   spatial : Q1 -> Q2 -> T1 -> T2 scan -> [host learns total] -> T3 traversal (fill)
+//   knn     : Q1 -> Q2 -> K1 traversal + K2 emit
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <mutex>
+
+#include "common.cuh"
+
+namespace arbx {
+
+std::atomic<long long> g_launches{0};
+static thread_local char t_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(t_err, sizeof(t_err), fmt, ap);
+  va_end(ap);
+}
+
+static std::once_flag g_pool_once[64];
+
+arbx_status scratch_alloc(void** p, size_t bytes, cudaStream_t s) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev >= 0 && dev < 64) {
+    // keep freed scratch cached in the stream-ordered pool instead of returning it to the OS
+    std::call_once(g_pool_once[dev], [dev] {
+      cudaMemPool_t pool;
+      if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        unsigned long long thr = ~0ull;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+      }
+    });
+  }
+  *p = nullptr;
+  cudaError_t e = cudaMallocAsync(p, bytes ? bytes : 1, s);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    set_error("cudaMallocAsync(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? ARBX_ERR_OOM : ARBX_ERR_CUDA;
+  }
+  return ARBX_OK;
+}
+void scratch_free(void* p, cudaStream_t s) { if (p) cudaFreeAsync(p, s); }
+
+const DimTable* dim_table_1(); const DimTable* dim_table_2(); const DimTable* dim_table_3();
+const DimTable* dim_table_4(); const DimTable* dim_table_5(); const DimTable* dim_table_6();
+const DimTable* dim_table_7(); const DimTable* dim_table_8(); const DimTable* dim_table_9();
+const DimTable* dim_table_10();
+
+const DimTable* dim_table(int dim) {
+  switch (dim) {
+    case 1: return dim_table_1(); case 2: return dim_table_2(); case 3: return dim_table_3();
+    case 4: return dim_table_4(); case 5: return dim_table_5(); case 6: return dim_table_6();
+    case 7: return dim_table_7(); case 8: return dim_table_8(); case 9: return dim_table_9();
+    case 10: return dim_table_10();
+  }
+  return nullptr;
+}
+
+static int env_int(const char* name, int dflt) {
+  const char* v = getenv(name);
+  return v && *v ? atoi(v) : dflt;
+}
+
+static void free_index(Index* ix, cudaStream_t s) {
+  scratch_free(ix->leaves, s); scratch_free(ix->nodes, s); scratch_free(ix->bounds, s);
+  scratch_free(ix->root, s); scratch_free(ix->codes, s);
+}
+
+// Q1 + Q2: order in which the queries are traversed (neighbours on the curve share a warp)
+static arbx_status query_order(const Index* ix, const float* queries, int64_t nq, int qkind,
+                               Scratch<uint32_t>& order, cudaStream_t s) {
+  Scratch<uint32_t> codes;
+  ARBX_TRY(codes.alloc((size_t)nq, s));
+  ARBX_TRY(order.alloc((size_t)nq, s));
+  int key_bits = 32;
+  ARBX_TRY(dim_table(ix->dim)->qcode(ix, queries, nq, qkind, codes.p, &key_bits, s));
+  return radix_sort_u32(codes.p, order.p, true, nq, key_bits, s);
+}
+
+__global__ void fill_i32_kernel(int32_t* p, int64_t n, int32_t v) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = v;
+}
+__global__ void fill_knn_empty_kernel(int32_t* idx, float* dist, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    idx[i] = -1;
+    if (dist) dist[i] = INFINITY;
+  }
+}
+
+}  // namespace arbx
+
+using namespace arbx;
+
+struct arbx_index_s { Index ix; };
+
+static bool bad_kind(int k) { return k < 0 || k > 2; }
+constexpr int64_t kMaxCount = int64_t(1) << 30;
+
+extern "C" {
+
+arbx_status arbx_build(const float* prims, int64_t n, int dim, arbx_kind kind, arbx_stream stream,
+                       arbx_handle* out) {
+  if (!out || n < 0 || dim < 1 || dim > ARBX_MAX_DIM || bad_kind((int)kind) || (n > 0 && !prims)) {
+    set_error("arbx_build: invalid argument (n=%lld dim=%d kind=%d)", (long long)n, dim, (int)kind);
+    return ARBX_ERR_INVALID_ARG;
+  }
+  if (n > kMaxCount) { set_error("arbx_build: n > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
+  cudaStream_t s = (cudaStream_t)stream;
+  arbx_index_s* h = new arbx_index_s();
+  h->ix.leaf_max = std::max(1, std::min(64, env_int("ARBX_LEAF_MAX", 4)));
+  arbx_status st = build_index(prims, n, dim, (int)kind, s, &h->ix);
+  if (st != ARBX_OK) {
+    free_index(&h->ix, s);
+    delete h;
+    return st;
+  }
+  *out = h;
+  return ARBX_OK;
+}
+
+arbx_status arbx_destroy(arbx_handle h, arbx_stream stream) {
+  if (!h) return ARBX_OK;
+  free_index(&h->ix, (cudaStream_t)stream);
+  delete h;
+  return ARBX_OK;
+}
+
+arbx_status arbx_size(arbx_handle h, int64_t* n) {
+  if (!h || !n) { set_error("arbx_size: null argument"); return ARBX_ERR_INVALID_ARG; }
+  *n = h->ix.n;
+  return ARBX_OK;
+}
+
+arbx_status arbx_bounds(arbx_handle h, float* lo_host, float* hi_host, arbx_stream stream) {
+  if (!h || !lo_host || !hi_host) { set_error("arbx_bounds: null argument"); return ARBX_ERR_INVALID_ARG; }
+  cudaStream_t s = (cudaStream_t)stream;
+  float tmp[2 * ARBX_MAX_DIM];
+  const int D = h->ix.dim;
+  ARBX_CUDA(cudaMemcpyAsync(tmp, h->ix.bounds, 2 * D * sizeof(float), cudaMemcpyDeviceToHost, s));
+  ARBX_CUDA(cudaStreamSynchronize(s));
+  for (int a = 0; a < D; ++a) { lo_host[a] = tmp[a]; hi_host[a] = tmp[D + a]; }
+  return ARBX_OK;
+}
+
+arbx_status arbx_query_count(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                             int32_t* counts, arbx_stream stream) {
+  if (!h || nq < 0 || bad_kind((int)qkind) || (nq > 0 && (!queries || !counts))) {
+    set_error("arbx_query_count: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  if (nq > kMaxCount) { set_error("arbx_query_count: nq > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
+  if (nq == 0) return ARBX_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  const Index* ix = &h->ix;
+  if (ix->n == 0) { ARBX_CUDA(cudaMemsetAsync(counts, 0, (size_t)nq * sizeof(int32_t), s)); return ARBX_OK; }
+  Scratch<uint32_t> order;
+  ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
+  return dim_table(ix->dim)->spatial(ix, queries, nq, (int)qkind, order.p, counts, nullptr, nullptr, s);
+}
+
+arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                               int32_t* offsets, int32_t* indices, int64_t indices_capacity,
+                               int64_t* total_host, arbx_stream stream) {
+  if (!h || nq < 0 || bad_kind((int)qkind) || !offsets || (nq > 0 && !queries) || indices_capacity < 0) {
+    set_error("arbx_query_spatial: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  if (nq > kMaxCount) { set_error("arbx_query_spatial: nq > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
+  cudaStream_t s = (cudaStream_t)stream;
+  const Index* ix = &h->ix;
+  if (total_host) *total_host = 0;
+  if (nq == 0 || ix->n == 0) {
+    ARBX_CUDA(cudaMemsetAsync(offsets, 0, (size_t)(nq + 1) * sizeof(int32_t), s));
+    return ARBX_OK;
+  }
+  Scratch<uint32_t> order;
+  Scratch<int32_t> counts;
+  Scratch<long long> total_dev;
+  ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
+  ARBX_TRY(counts.alloc((size_t)nq, s));
+  ARBX_TRY(total_dev.alloc(1, s));
+  const DimTable* tab = dim_table(ix->dim);
+  ARBX_TRY(tab->spatial(ix, queries, nq, (int)qkind, order.p, counts.p, nullptr, nullptr, s));
+  ARBX_TRY(exclusive_scan_i32(counts.p, offsets, nq, total_dev.p, s));
+  long long total = 0;
+  ARBX_CUDA(cudaMemcpyAsync(&total, total_dev.p, sizeof(total), cudaMemcpyDeviceToHost, s));
+  ARBX_CUDA(cudaStreamSynchronize(s));
+  if (total_host) *total_host = total;
+  if (total > 0x7fffffffLL) {
+    set_error("arbx_query_spatial: total %lld exceeds INT32_MAX", total);
+    return ARBX_ERR_OVERFLOW;
+  }
+  if (!indices) return ARBX_OK;
+  if (indices_capacity < total) {
+    set_error("arbx_query_spatial: capacity %lld < total %lld", (long long)indices_capacity, total);
+    return ARBX_ERR_CAPACITY;
+  }
+  if (total == 0) return ARBX_OK;
+  return tab->spatial(ix, queries, nq, (int)qkind, order.p, nullptr, offsets, indices, s);
+}
+
+arbx_status arbx_query_knn(arbx_handle h, const float* qpoints, int64_t nq, int k, int32_t* indices,
+                           float* distances, arbx_stream stream) {
+  if (!h || nq < 0 || k < 1 || (nq > 0 && (!qpoints || !indices))) {
+    set_error("arbx_query_knn: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  if (k > ARBX_K_MAX) { set_error("arbx_query_knn: k=%d > ARBX_K_MAX=%d", k, ARBX_K_MAX); return ARBX_ERR_UNSUPPORTED; }
+  if (nq > kMaxCount) { set_error("arbx_query_knn: nq > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
+  if (nq == 0) return ARBX_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  const Index* ix = &h->ix;
+  if (ix->n == 0) {
+    fill_knn_empty_kernel<<<256, 256, 0, s>>>(indices, distances, nq * k);
+    ARBX_LAUNCH_CHECK();
+    return ARBX_OK;
+  }
+  Scratch<uint32_t> order;
+  ARBX_TRY(query_order(ix, qpoints, nq, KIND_POINT, order, s));
+  return dim_table(ix->dim)->knn(ix, qpoints, nq, k, order.p, indices, distances, s);
+}
+
+arbx_status arbx_sort_pairs(void* keys, uint32_t* values, int64_t n, int key_bytes, int key_bits,
+                            arbx_stream stream) {
+  if (n < 0 || (n > 0 && !keys) || (key_bytes != 4 && key_bytes != 8) || key_bits < 1 || key_bits > 8 * key_bytes) {
+    set_error("arbx_sort_pairs: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  if (key_bytes == 8) return radix_sort_u64((unsigned long long*)keys, values, false, n, key_bits, s);
+  return radix_sort_u32((uint32_t*)keys, values, false, n, key_bits, s);
+}
+
+arbx_status arbx_debug_validate(arbx_handle h, int64_t* violations_host, arbx_stream stream) {
+  if (!h || !violations_host) { set_error("arbx_debug_validate: null argument"); return ARBX_ERR_INVALID_ARG; }
+  return validate_index(&h->ix, violations_host, (cudaStream_t)stream);
+}
+
+int64_t arbx_launch_count(void) { return (int64_t)g_launches.load(); }
+
+const char* arbx_status_string(arbx_status s) {
+  switch (s) {
+    case ARBX_OK: return "ARBX_OK";
+    case ARBX_ERR_INVALID_ARG: return "ARBX_ERR_INVALID_ARG";
+    case ARBX_ERR_UNSUPPORTED: return "ARBX_ERR_UNSUPPORTED";
+    case ARBX_ERR_CAPACITY: return "ARBX_ERR_CAPACITY";
+    case ARBX_ERR_OVERFLOW: return "ARBX_ERR_OVERFLOW";
+    case ARBX_ERR_CUDA: return "ARBX_ERR_CUDA";
+    case ARBX_ERR_OOM: return "ARBX_ERR_OOM";
+  }
+  return "ARBX_ERR_UNKNOWN";
+}
+
+const char* arbx_last_error(void) { return t_err; }
+
+}  // extern "C"

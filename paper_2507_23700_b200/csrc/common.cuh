@@ -1,0 +1,125 @@
+// common.cuh -- shared declarations of the CUDA path (sm_100a).  Internal, not part of the ABI.
+//
+// Data layout in HBM:
+//   leaves : sorted (space-filling-curve order) array, one record per primitive, stride
+//            LEAF_W floats (multiple of 4 => every record is 16-byte aligned, LDG.128):
+//              POINT  x[D], idx            (D=3: 16 B, the paper's 16-byte leaf)
+//              BOX    lo[D], hi[D], idx
+//              SPHERE c[D], R, idx
+//            idx = position in the caller's array; bit 31 set marks the LAST record of a
+//            leaf range (a collapsed subtree of <= leaf_max primitives).
+//   nodes  : one record per internal node, id = split position s (between sorted leaves s and
+//            s+1), stride 4*(D+1) floats:  lo0[D], hi0[D], lo1[D], hi1[D], c0, c1, pad, pad.
+//            A node stores the boxes of its TWO CHILDREN, so one fetch decides both descents.
+//            child ref c >= 0: internal node id; c < 0: leaf range starting at leaf ~c.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+
+#include "../../include/arbx.h"
+
+namespace arbx {
+
+constexpr int KIND_POINT = 0, KIND_BOX = 1, KIND_SPHERE = 2;
+constexpr uint32_t LEAF_END = 0x80000000u;
+constexpr int STACK_DEPTH = 96;   // <= 64 code bits + 31 index tie-break bits + 1
+
+__host__ __device__ constexpr int prim_width(int kind, int D) {
+  return kind == KIND_POINT ? D : kind == KIND_BOX ? 2 * D : D + 1;
+}
+__host__ __device__ constexpr int leaf_width(int kind, int D) {
+  return (prim_width(kind, D) + 1 + 3) / 4 * 4;
+}
+__host__ __device__ constexpr int node_width(int D) { return 4 * (D + 1); }
+
+struct Index {
+  int64_t n = 0;
+  int dim = 0;
+  int kind = 0;
+  int leaf_max = 1;
+  float* leaves = nullptr;      // n * leaf_width floats
+  float* nodes = nullptr;       // max(n-1,0) * node_width floats
+  float* bounds = nullptr;      // 2*dim floats: lo[dim], hi[dim] of all primitives
+  int32_t* root = nullptr;      // 1 int: root child ref (device)
+  unsigned long long* codes = nullptr;  // sorted codes, kept only for arbx_debug_validate
+};
+
+// ---- error plumbing ----------------------------------------------------------------------
+void set_error(const char* fmt, ...);
+extern std::atomic<long long> g_launches;
+inline void count_launch(int k = 1) { g_launches.fetch_add(k, std::memory_order_relaxed); }
+
+#define ARBX_CUDA(expr)                                                                  \
+  do {                                                                                   \
+    cudaError_t e__ = (expr);                                                            \
+    if (e__ != cudaSuccess) {                                                            \
+      ::arbx::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, \
+                        __LINE__);                                                       \
+      return e__ == cudaErrorMemoryAllocation ? ARBX_ERR_OOM : ARBX_ERR_CUDA;            \
+    }                                                                                    \
+  } while (0)
+
+#define ARBX_LAUNCH_CHECK()                                                              \
+  do {                                                                                   \
+    ::arbx::count_launch();                                                              \
+    ARBX_CUDA(cudaGetLastError());                                                       \
+  } while (0)
+
+#define ARBX_TRY(expr)                        \
+  do {                                        \
+    arbx_status s__ = (expr);                 \
+    if (s__ != ARBX_OK) return s__;           \
+  } while (0)
+
+// stream-ordered scratch (never stored in the handle)
+arbx_status scratch_alloc(void** p, size_t bytes, cudaStream_t s);
+void scratch_free(void* p, cudaStream_t s);
+
+template <class T>
+struct Scratch {   // RAII: released in stream order when the call returns
+  T* p = nullptr;
+  cudaStream_t s = nullptr;
+  Scratch() = default;
+  Scratch(const Scratch&) = delete;
+  Scratch& operator=(const Scratch&) = delete;
+  ~Scratch() { if (p) scratch_free(p, s); }
+  arbx_status alloc(size_t count, cudaStream_t stream) {
+    s = stream;
+    return scratch_alloc((void**)&p, (count ? count : 1) * sizeof(T), stream);
+  }
+  T* release() { T* q = p; p = nullptr; return q; }
+};
+
+// ---- internal entry points (one per translation unit) --------------------------------------
+// sort.cu: stable LSD radix sort of bits [0,key_bits).  vals_in == nullptr means "value =
+// position" (saves writing and re-reading an iota).  Result is left in keys/vals (in place
+// from the caller's point of view; ping-pong scratch is internal).
+arbx_status radix_sort_u64(unsigned long long* keys, uint32_t* vals, bool iota_vals, int64_t n,
+                           int key_bits, cudaStream_t s);
+arbx_status radix_sort_u32(uint32_t* keys, uint32_t* vals, bool iota_vals, int64_t n,
+                           int key_bits, cudaStream_t s);
+
+// build.cu
+arbx_status build_index(const float* prims, int64_t n, int dim, int kind, cudaStream_t s,
+                        Index* ix);
+arbx_status validate_index(const Index* ix, int64_t* violations_host, cudaStream_t s);
+
+// query_dN.cu (one TU per dimension), dispatched from query.cu
+using spatial_fn = arbx_status (*)(const Index*, const float* queries, int64_t nq, int qkind,
+                                   const uint32_t* qorder, int32_t* counts,
+                                   const int32_t* offsets, int32_t* indices, cudaStream_t);
+using knn_fn = arbx_status (*)(const Index*, const float* qpoints, int64_t nq, int k,
+                               const uint32_t* qorder, int32_t* indices, float* distances,
+                               cudaStream_t);
+using qcode_fn = arbx_status (*)(const Index*, const float* queries, int64_t nq, int qkind_or_point,
+                                 uint32_t* codes, int* key_bits, cudaStream_t);
+struct DimTable { spatial_fn spatial; knn_fn knn; qcode_fn qcode; };
+const DimTable* dim_table(int dim);
+
+// scan.cu: offsets[0..nq] = exclusive scan of counts[0..nq); *total (device, int64) = sum
+arbx_status exclusive_scan_i32(const int32_t* counts, int32_t* offsets, int64_t nq,
+                               long long* total_dev, cudaStream_t s);
+
+}  // namespace arbx

@@ -1,0 +1,435 @@
+// query_dim.cu -- compiled once per dimension (-DARBX_DIM=1..10): query steps Q1 (query codes),
+// T1/T3 (spatial traversal: count / fill) and K1/K2 (kNN traversal + emit).  SURVEY.md §8(a).
+// PAPER.md:L69 (radius / nearest predicates), L79 (nearest = distance to the stored geometry),
+// L104-115 (callback / storage queries), L295 + L307 (traversal, sorted queries), L303 (count).
+//
+// One query per thread; the 32 queries of a warp are neighbours on the space-filling curve
+// (qorder), so they walk nearly the same nodes and the node fetches hit L1/L2.
+#include <algorithm>
+
+#include "geom.cuh"
+
+#ifndef ARBX_DIM
+#error "compile with -DARBX_DIM=<1..10>"
+#endif
+
+namespace arbx {
+namespace {
+
+constexpr int D = ARBX_DIM;
+constexpr int QT = 128;   // threads per block of the traversal kernels
+
+// ---- Q1: 32-bit space-filling code of each query centre inside the scene bounds --------------
+template <int QK>
+__global__ void __launch_bounds__(256) qcode_kernel(const float* __restrict__ queries, int64_t nq,
+                                                    const float* __restrict__ bounds,
+                                                    uint32_t* __restrict__ codes) {
+  constexpr int QW = prim_width(QK, D);
+  constexpr int B = qcode_bits_per_axis(D);
+  float lo[D], scale[D];
+#pragma unroll
+  for (int a = 0; a < D; ++a) {
+    lo[a] = bounds[a];
+    float ext = bounds[D + a] - lo[a];
+    scale[a] = ext > 0.f ? exp2f((float)B) / ext : 0.f;
+  }
+  for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < nq; i += (int64_t)gridDim.x * 256) {
+    float v[QW], c[D];
+#pragma unroll
+    for (int e = 0; e < QW; ++e) v[e] = __ldg(queries + i * QW + e);
+    centre_of<D, QK>(v, c);
+    uint32_t q[D];
+    quantise<D, B>(c, lo, scale, q);
+    codes[i] = interleave<D, B, uint32_t>(q);
+  }
+}
+
+// ---- node / leaf access ------------------------------------------------------------------------
+struct Node { float v[4 * D]; int32_t c0, c1; };
+
+__device__ __forceinline__ void load_node(const float4* __restrict__ nodes, int32_t ref, Node& nd) {
+  const float4* p = nodes + (int64_t)ref * (D + 1);
+#pragma unroll
+  for (int e = 0; e < D; ++e) {
+    float4 t = __ldg(p + e);
+    nd.v[4 * e] = t.x; nd.v[4 * e + 1] = t.y; nd.v[4 * e + 2] = t.z; nd.v[4 * e + 3] = t.w;
+  }
+  float4 t = __ldg(p + D);
+  nd.c0 = __float_as_int(t.x);
+  nd.c1 = __float_as_int(t.y);
+}
+
+template <int PK>
+struct Leaf { float v[prim_width(PK, D)]; uint32_t idx; };
+
+template <int PK>
+__device__ __forceinline__ void load_leaf(const float4* __restrict__ leaves, int j, Leaf<PK>& lf) {
+  constexpr int W = prim_width(PK, D);
+  constexpr int LW = leaf_width(PK, D);
+  float t[LW];
+  const float4* p = leaves + (int64_t)j * (LW / 4);
+#pragma unroll
+  for (int e = 0; e < LW / 4; ++e) {
+    float4 x = __ldg(p + e);
+    t[4 * e] = x.x; t[4 * e + 1] = x.y; t[4 * e + 2] = x.z; t[4 * e + 3] = x.w;
+  }
+#pragma unroll
+  for (int e = 0; e < W; ++e) lf.v[e] = t[e];
+  lf.idx = __float_as_uint(t[W]);
+}
+
+// ---- spatial predicates (closed sets) ---------------------------------
+template <int QK>
+struct Query {
+  float v[prim_width(QK, D)];
+  float r2;   // SPHERE: r*r
+};
+
+template <int QK>
+__device__ __forceinline__ bool hits_box(const Query<QK>& q, const float* lo, const float* hi) {
+  if constexpr (QK == KIND_SPHERE) {
+    return dist2_pb<D>(q.v, lo, hi) <= q.r2;
+  } else if constexpr (QK == KIND_BOX) {
+    bool ok = true;
+#pragma unroll
+    for (int a = 0; a < D; ++a) ok = ok && lo[a] <= q.v[D + a] && q.v[a] <= hi[a];
+    return ok;
+  } else {
+    bool ok = true;
+#pragma unroll
+    for (int a = 0; a < D; ++a) ok = ok && lo[a] <= q.v[a] && q.v[a] <= hi[a];
+    return ok;
+  }
+}
+
+template <int QK, int PK>
+__device__ __forceinline__ bool hits_prim(const Query<QK>& q, const float* p) {
+  if constexpr (PK == KIND_BOX) {
+    return hits_box<QK>(q, p, p + D);
+  } else if constexpr (PK == KIND_POINT) {
+    if constexpr (QK == KIND_SPHERE) {
+      return dist2_pp<D>(p, q.v) <= q.r2;
+    } else if constexpr (QK == KIND_BOX) {
+      bool ok = true;
+#pragma unroll
+      for (int a = 0; a < D; ++a) ok = ok && q.v[a] <= p[a] && p[a] <= q.v[D + a];
+      return ok;
+    } else {
+      bool ok = true;
+#pragma unroll
+      for (int a = 0; a < D; ++a) ok = ok && p[a] == q.v[a];
+      return ok;
+    }
+  } else {   // SPHERE primitive (c, R)
+    const float R = p[D];
+    if constexpr (QK == KIND_SPHERE) {
+      const float rr = q.v[D] + R;
+      return dist2_pp<D>(p, q.v) <= rr * rr;
+    } else if constexpr (QK == KIND_BOX) {
+      return dist2_pb<D>(p, q.v, q.v + D) <= R * R;
+    } else {
+      return dist2_pp<D>(q.v, p) <= R * R;
+    }
+  }
+}
+
+// ---- T1 / T3: spatial traversal ------------------------------------------------------------------
+template <int PK, int QK, bool FILL>
+__global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ nodes,
+                                                     const float4* __restrict__ leaves,
+                                                     const int32_t* __restrict__ root,
+                                                     const float* __restrict__ queries,
+                                                     const uint32_t* __restrict__ qorder, int64_t nq,
+                                                     int32_t* __restrict__ counts,
+                                                     const int32_t* __restrict__ offsets,
+                                                     int32_t* __restrict__ indices) {
+  constexpr int QW = prim_width(QK, D);
+  const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
+  if (t >= nq) return;
+  const int64_t qi = qorder ? (int64_t)qorder[t] : t;
+  Query<QK> q;
+#pragma unroll
+  for (int e = 0; e < QW; ++e) q.v[e] = __ldg(queries + qi * QW + e);
+  bool alive = true;
+  if constexpr (QK == KIND_SPHERE) {
+    q.r2 = q.v[D] * q.v[D];
+    alive = q.v[D] >= 0.f;      // negative radius matches nothing (reading A21)
+  }
+  int32_t* out = nullptr;
+  if constexpr (FILL) out = indices + offsets[qi];
+  int cnt = 0;
+  if (alive) {
+    int32_t stack[STACK_DEPTH];
+    int sp = 0;
+    int32_t ref = __ldg(root);
+    for (;;) {
+      if (ref >= 0) {
+        Node nd;
+        load_node(nodes, ref, nd);
+        const bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
+        const bool h1 = hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D);
+        if (h0) {
+          ref = nd.c0;
+          if (h1) stack[sp++] = nd.c1;
+          continue;
+        }
+        if (h1) { ref = nd.c1; continue; }
+      } else {
+        int j = ~ref;
+        for (;; ++j) {
+          Leaf<PK> lf;
+          load_leaf<PK>(leaves, j, lf);
+          if (hits_prim<QK, PK>(q, lf.v)) {
+            if constexpr (FILL) out[cnt] = (int32_t)(lf.idx & ~LEAF_END);
+            ++cnt;
+          }
+          if (lf.idx & LEAF_END) break;
+        }
+      }
+      if (sp == 0) break;
+      ref = stack[--sp];
+    }
+  }
+  if constexpr (!FILL) counts[qi] = cnt;
+}
+
+// ---- K1 / K2: k nearest neighbours ------------------------------------------------------------------
+// Heap key: squared distance for POINT/BOX primitives, distance for SPHERE primitives
+// (max(0,||y-c||-R) is not monotone in the squared centre distance alone).
+template <int PK>
+__device__ __forceinline__ float knn_key(const float* y, const float* p) {
+  if constexpr (PK == KIND_POINT) return dist2_pp<D>(p, y);
+  else if constexpr (PK == KIND_BOX) return dist2_pb<D>(y, p, p + D);
+  else return fmaxf(0.f, sqrtf(dist2_pp<D>(p, y)) - p[D]);
+}
+template <int PK>
+__device__ __forceinline__ float knn_bound(const float* y, const float* lo, const float* hi) {
+  const float d2 = dist2_pb<D>(y, lo, hi);
+  if constexpr (PK == KIND_SPHERE) return sqrtf(d2);
+  else return d2;
+}
+
+// Best-k container, KB > 0: ascending sorted array in registers (all indices static).  Slots
+// [0, KB-k) hold -inf sentinels so that the k-th best is always slot KB-1.
+template <int KB>
+struct RegHeap {
+  float d[KB];
+  int32_t i[KB];
+  __device__ __forceinline__ void init(int k) {
+#pragma unroll
+    for (int s = 0; s < KB; ++s) { d[s] = s < KB - k ? -INFINITY : INFINITY; i[s] = -1; }
+  }
+  __device__ __forceinline__ float worst() const { return d[KB - 1]; }
+  __device__ __forceinline__ void push(float t, int32_t idx) {   // requires t < worst()
+    d[KB - 1] = t; i[KB - 1] = idx;
+#pragma unroll
+    for (int s = KB - 1; s > 0; --s) {
+      const bool sw = d[s] < d[s - 1];
+      const float td = d[s]; const int32_t ti = i[s];
+      d[s] = sw ? d[s - 1] : td; i[s] = sw ? i[s - 1] : ti;
+      d[s - 1] = sw ? td : d[s - 1]; i[s - 1] = sw ? ti : i[s - 1];
+    }
+  }
+  template <class F>
+  __device__ __forceinline__ void emit(int k, F&& f) {
+#pragma unroll
+    for (int s = 0; s < KB; ++s)
+      if (s >= KB - k) f(s - (KB - k), d[s], i[s]);
+  }
+};
+
+// k > 32: binary max-heap in local memory, heap-sorted at the end
+struct LocalHeap {
+  float d[ARBX_K_MAX];
+  int32_t i[ARBX_K_MAX];
+  int k, m;
+  __device__ __forceinline__ void init(int k_) { k = k_; m = 0; }
+  __device__ __forceinline__ float worst() const { return m < k ? INFINITY : d[0]; }
+  __device__ __forceinline__ void sift_down(int pos, int size, float t, int32_t idx) {
+    for (;;) {
+      int c = 2 * pos + 1;
+      if (c >= size) break;
+      if (c + 1 < size && d[c + 1] > d[c]) ++c;
+      if (d[c] <= t) break;
+      d[pos] = d[c]; i[pos] = i[c];
+      pos = c;
+    }
+    d[pos] = t; i[pos] = idx;
+  }
+  __device__ __forceinline__ void push(float t, int32_t idx) {
+    if (m < k) {
+      int pos = m++;
+      while (pos > 0) {
+        int par = (pos - 1) >> 1;
+        if (d[par] >= t) break;
+        d[pos] = d[par]; i[pos] = i[par];
+        pos = par;
+      }
+      d[pos] = t; i[pos] = idx;
+    } else {
+      sift_down(0, k, t, idx);
+    }
+  }
+  template <class F>
+  __device__ __forceinline__ void emit(int kk, F&& f) {
+    for (int size = m; size > 1; --size) {   // heap sort: largest to the back
+      const float t = d[size - 1]; const int32_t idx = i[size - 1];
+      d[size - 1] = d[0]; i[size - 1] = i[0];
+      sift_down(0, size - 1, t, idx);
+    }
+    for (int s = 0; s < kk; ++s) f(s, s < m ? d[s] : INFINITY, s < m ? i[s] : -1);
+  }
+};
+
+template <int PK, class Heap>
+__global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ nodes,
+                                                 const float4* __restrict__ leaves,
+                                                 const int32_t* __restrict__ root,
+                                                 const float* __restrict__ qpoints,
+                                                 const uint32_t* __restrict__ qorder, int64_t nq, int k,
+                                                 int64_t n, int32_t* __restrict__ indices,
+                                                 float* __restrict__ distances) {
+  const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
+  if (t >= nq) return;
+  const int64_t qi = qorder ? (int64_t)qorder[t] : t;
+  float y[D];
+#pragma unroll
+  for (int a = 0; a < D; ++a) y[a] = __ldg(qpoints + qi * D + a);
+  Heap heap;
+  heap.init(k);
+  if (n > 0) {
+    int32_t sref[STACK_DEPTH];
+    float sbound[STACK_DEPTH];
+    int sp = 0;
+    int32_t ref = __ldg(root);
+    for (;;) {
+      if (ref >= 0) {
+        Node nd;
+        load_node(nodes, ref, nd);
+        float b0 = knn_bound<PK>(y, nd.v, nd.v + D);
+        float b1 = knn_bound<PK>(y, nd.v + 2 * D, nd.v + 3 * D);
+        int32_t c0 = nd.c0, c1 = nd.c1;
+        if (b1 < b0) { float tb = b0; b0 = b1; b1 = tb; int32_t tc = c0; c0 = c1; c1 = tc; }
+        const float w = heap.worst();
+        if (b0 < w) {
+          ref = c0;
+          if (b1 < w) { sref[sp] = c1; sbound[sp] = b1; ++sp; }
+          continue;
+        }
+      } else {
+        int j = ~ref;
+        for (;; ++j) {
+          Leaf<PK> lf;
+          load_leaf<PK>(leaves, j, lf);
+          const float key = knn_key<PK>(y, lf.v);
+          if (key < heap.worst()) heap.push(key, (int32_t)(lf.idx & ~LEAF_END));
+          if (lf.idx & LEAF_END) break;
+        }
+      }
+      bool found = false;
+      while (sp > 0) {
+        --sp;
+        if (sbound[sp] < heap.worst()) { ref = sref[sp]; found = true; break; }
+      }
+      if (!found) break;
+    }
+  }
+  int32_t* oi = indices + qi * k;
+  float* od = distances ? distances + qi * k : nullptr;
+  heap.emit(k, [&](int s, float key, int32_t idx) {
+    oi[s] = idx;
+    if (od) od[s] = (PK == KIND_SPHERE || idx < 0) ? key : sqrtf(key);
+  });
+}
+
+// ---- host dispatch ------------------------------------------------------------------------------------
+template <int PK, int QK>
+arbx_status spatial_launch(const Index* ix, const float* queries, int64_t nq, const uint32_t* qorder,
+                           int32_t* counts, const int32_t* offsets, int32_t* indices, cudaStream_t s) {
+  const unsigned grid = (unsigned)((nq + QT - 1) / QT);
+  const float4* nodes = reinterpret_cast<const float4*>(ix->nodes);
+  const float4* leaves = reinterpret_cast<const float4*>(ix->leaves);
+  if (indices)
+    spatial_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
+  else
+    spatial_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
+  ARBX_LAUNCH_CHECK();
+  return ARBX_OK;
+}
+
+template <int PK>
+arbx_status spatial_pk(const Index* ix, const float* queries, int64_t nq, int qkind, const uint32_t* qorder,
+                       int32_t* counts, const int32_t* offsets, int32_t* indices, cudaStream_t s) {
+  switch (qkind) {
+    case KIND_POINT: return spatial_launch<PK, KIND_POINT>(ix, queries, nq, qorder, counts, offsets, indices, s);
+    case KIND_BOX: return spatial_launch<PK, KIND_BOX>(ix, queries, nq, qorder, counts, offsets, indices, s);
+    default: return spatial_launch<PK, KIND_SPHERE>(ix, queries, nq, qorder, counts, offsets, indices, s);
+  }
+}
+
+arbx_status spatial_entry(const Index* ix, const float* queries, int64_t nq, int qkind, const uint32_t* qorder,
+                          int32_t* counts, const int32_t* offsets, int32_t* indices, cudaStream_t s) {
+  switch (ix->kind) {
+    case KIND_POINT: return spatial_pk<KIND_POINT>(ix, queries, nq, qkind, qorder, counts, offsets, indices, s);
+    case KIND_BOX: return spatial_pk<KIND_BOX>(ix, queries, nq, qkind, qorder, counts, offsets, indices, s);
+    default: return spatial_pk<KIND_SPHERE>(ix, queries, nq, qkind, qorder, counts, offsets, indices, s);
+  }
+}
+
+template <int PK, class Heap>
+arbx_status knn_launch(const Index* ix, const float* qpoints, int64_t nq, int k, const uint32_t* qorder,
+                       int32_t* indices, float* distances, cudaStream_t s) {
+  const unsigned grid = (unsigned)((nq + QT - 1) / QT);
+  knn_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
+                                           reinterpret_cast<const float4*>(ix->leaves), ix->root, qpoints,
+                                           qorder, nq, k, ix->n, indices, distances);
+  ARBX_LAUNCH_CHECK();
+  return ARBX_OK;
+}
+
+template <int PK>
+arbx_status knn_pk(const Index* ix, const float* qpoints, int64_t nq, int k, const uint32_t* qorder,
+                   int32_t* indices, float* distances, cudaStream_t s) {
+  if (k <= 1) return knn_launch<PK, RegHeap<1>>(ix, qpoints, nq, k, qorder, indices, distances, s);
+  if (k <= 2) return knn_launch<PK, RegHeap<2>>(ix, qpoints, nq, k, qorder, indices, distances, s);
+  if (k <= 4) return knn_launch<PK, RegHeap<4>>(ix, qpoints, nq, k, qorder, indices, distances, s);
+  if (k <= 8) return knn_launch<PK, RegHeap<8>>(ix, qpoints, nq, k, qorder, indices, distances, s);
+  if (k <= 16) return knn_launch<PK, RegHeap<16>>(ix, qpoints, nq, k, qorder, indices, distances, s);
+  if (k <= 32) return knn_launch<PK, RegHeap<32>>(ix, qpoints, nq, k, qorder, indices, distances, s);
+  return knn_launch<PK, LocalHeap>(ix, qpoints, nq, k, qorder, indices, distances, s);
+}
+
+arbx_status knn_entry(const Index* ix, const float* qpoints, int64_t nq, int k, const uint32_t* qorder,
+                      int32_t* indices, float* distances, cudaStream_t s) {
+  switch (ix->kind) {
+    case KIND_POINT: return knn_pk<KIND_POINT>(ix, qpoints, nq, k, qorder, indices, distances, s);
+    case KIND_BOX: return knn_pk<KIND_BOX>(ix, qpoints, nq, k, qorder, indices, distances, s);
+    default: return knn_pk<KIND_SPHERE>(ix, qpoints, nq, k, qorder, indices, distances, s);
+  }
+}
+
+arbx_status qcode_entry(const Index* ix, const float* queries, int64_t nq, int qkind, uint32_t* codes,
+                        int* key_bits, cudaStream_t s) {
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((nq + 255) / 256, (int64_t)sms * 8));
+  switch (qkind) {
+    case KIND_POINT: qcode_kernel<KIND_POINT><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes); break;
+    case KIND_BOX: qcode_kernel<KIND_BOX><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes); break;
+    default: qcode_kernel<KIND_SPHERE><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes); break;
+  }
+  ARBX_LAUNCH_CHECK();
+  *key_bits = D * qcode_bits_per_axis(D);
+  return ARBX_OK;
+}
+
+const DimTable kTable = {spatial_entry, knn_entry, qcode_entry};
+
+}  // namespace
+
+#define ARBX_CAT2(a, b) a##b
+#define ARBX_CAT(a, b) ARBX_CAT2(a, b)
+const DimTable* ARBX_CAT(dim_table_, ARBX_DIM)() { return &kTable; }
+
+}  // namespace arbx

@@ -1,0 +1,101 @@
+// scan.cu -- query step T2: offsets = exclusive prefix sum of per-query counts (CSR offsets,
+// PAPER.md:L69 "offsets").  Totals are carried in 64 bits so that a result
+// larger than INT32_MAX is detected instead of wrapping (reading A11).
+#include <algorithm>
+
+#include "common.cuh"
+
+namespace arbx {
+namespace {
+
+constexpr int ST = 256, SI = 8, SB = ST * SI;   // 2048 counts per block
+
+__device__ __forceinline__ long long block_exclusive_scan(long long v, long long* total) {
+  __shared__ long long wsum[ST / 32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  long long x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    long long y = __shfl_up_sync(~0u, x, o);
+    if (lane >= o) x += y;
+  }
+  if (lane == 31) wsum[w] = x;
+  __syncthreads();
+  long long base = 0, tot = 0;
+#pragma unroll
+  for (int i = 0; i < ST / 32; ++i) { if (i < w) base += wsum[i]; tot += wsum[i]; }
+  *total = tot;
+  __syncthreads();
+  return base + x - v;
+}
+
+__global__ void __launch_bounds__(ST) block_sums_kernel(const int32_t* __restrict__ counts, int64_t nq,
+                                                        long long* __restrict__ sums) {
+  const int64_t base = (int64_t)blockIdx.x * SB + (int64_t)threadIdx.x * SI;
+  long long v = 0;
+#pragma unroll
+  for (int e = 0; e < SI; ++e) if (base + e < nq) v += counts[base + e];
+  long long tot;
+  block_exclusive_scan(v, &tot);
+  if (threadIdx.x == 0) sums[blockIdx.x] = tot;
+}
+
+// single block: exclusive scan of the block sums in place, grand total to *total
+__global__ void __launch_bounds__(ST) scan_sums_kernel(long long* sums, int nb, long long* total) {
+  long long carry = 0;
+  for (int b0 = 0; b0 < nb; b0 += ST) {
+    const int i = b0 + threadIdx.x;
+    long long v = i < nb ? sums[i] : 0, tot;
+    long long ex = block_exclusive_scan(v, &tot);
+    if (i < nb) sums[i] = carry + ex;
+    carry += tot;
+  }
+  if (threadIdx.x == 0) *total = carry;
+}
+
+__global__ void __launch_bounds__(ST) apply_kernel(const int32_t* __restrict__ counts, int64_t nq,
+                                                   const long long* __restrict__ sums,
+                                                   const long long* __restrict__ total,
+                                                   int32_t* __restrict__ offsets) {
+  const int64_t base = (int64_t)blockIdx.x * SB + (int64_t)threadIdx.x * SI;
+  int32_t c[SI];
+  long long v = 0;
+#pragma unroll
+  for (int e = 0; e < SI; ++e) { c[e] = base + e < nq ? counts[base + e] : 0; v += c[e]; }
+  long long tot;
+  long long run = sums[blockIdx.x] + block_exclusive_scan(v, &tot);
+#pragma unroll
+  for (int e = 0; e < SI; ++e) {
+    if (base + e < nq) offsets[base + e] = (int32_t)run;
+    run += c[e];
+  }
+  if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
+    const long long t = *total;
+    offsets[nq] = t > 0x7fffffffLL ? 0x7fffffff : (int32_t)t;
+  }
+}
+
+__global__ void zero_total_kernel(int32_t* offsets, long long* total) { offsets[0] = 0; *total = 0; }
+
+}  // namespace
+
+arbx_status exclusive_scan_i32(const int32_t* counts, int32_t* offsets, int64_t nq, long long* total_dev,
+                               cudaStream_t s) {
+  if (nq == 0) {
+    zero_total_kernel<<<1, 1, 0, s>>>(offsets, total_dev);
+    ARBX_LAUNCH_CHECK();
+    return ARBX_OK;
+  }
+  const int nb = (int)((nq + SB - 1) / SB);
+  Scratch<long long> sums;
+  ARBX_TRY(sums.alloc(nb, s));
+  block_sums_kernel<<<nb, ST, 0, s>>>(counts, nq, sums.p);
+  ARBX_LAUNCH_CHECK();
+  scan_sums_kernel<<<1, ST, 0, s>>>(sums.p, nb, total_dev);
+  ARBX_LAUNCH_CHECK();
+  apply_kernel<<<nb, ST, 0, s>>>(counts, nq, sums.p, total_dev, offsets);
+  ARBX_LAUNCH_CHECK();
+  return ARBX_OK;
+}
+
+}  // namespace arbx
