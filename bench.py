@@ -1,0 +1,431 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hot path of arXiv 2507.23700 on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C3]
+
+A STEP is one pass of the whole hot path (every row of SURVEY.md §8(a)) over one synthetic
+batch, through the C ABI:
+    arbx_build(N prims)                      B1..B6
+    arbx_query_spatial(Q queries) -> CSR     Q1,Q2,T1,T2,T3
+    arbx_query_count(Q queries)              Q1,Q2,T1 (= T4, the count-only callback path)
+    arbx_query_knn(Q points, k)              Q1,Q2,K1,K2      (when the workload has a k)
+    arbx_destroy
+The default workload is BASELINE.json configs[2] ("C3": N = Q = 10^7 3-D fp32 points, hollow
+sphere queries, radius with ~16 neighbours, kNN k = 16) -- the configuration BASELINE.json's
+metric is quoted on ("... at N=10M fp32 3D").
+
+value       = queries answered per second over the whole step (3 query batches; the build
+              is inside the step), inputs resident in HBM, device-timed.
+e2e         = the same with pinned-HOST inputs copied to the device and every result copied
+              back to pinned host memory inside the timed region.
+breakdown   = per-call rates: build Mprims/s, radius/count/kNN queries/s, and per hot-path
+              step milliseconds + achieved algorithmic GB/s (arbx_profile_*, CUDA events).
+roofline    = the dominant kernel (largest share of the step) against the measured HBM peak.
+cpu_baseline= the oracle (oracle/, never tuned) on the host cores, bounded sample.
+
+N > 1 (torchrun): replicas only -- every rank runs the same step on its own data (rank
+seeds), no data-path collective; value = all ranks' queries / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "BVH build Mprims/s; radius & kNN(k=16) queries/s at N=10M fp32 3D; HBM GB/s"
+UNIT = "queries/s"
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---- algorithmic HBM bytes per hot-path step ----------
+def algorithmic_bytes(cfg, totals):
+    """Bytes the method itself must move per step, per kernel id of arbx_profile_kernel_name."""
+    n, nq, D = cfg["n"], cfg["nq"], cfg["dim"]
+    pk, qk = cfg["pkind"], cfg["qkind"]
+    pw = D if pk == 0 else 2 * D if pk == 1 else D + 1          # floats per primitive row
+    qw = D if qk == 0 else 2 * D if qk == 1 else D + 1          # floats per spatial query row
+    lw = (pw + 1 + 3) // 4 * 4                                  # floats per leaf record
+    nw = 4 * (D + 1)                                            # floats per internal node
+    npass = (D * min(32, 64 // D) + 7) // 8                     # 8-bit digit passes, build sort
+    qpass = (D * min(16, 32 // D) + 7) // 8                     # 8-bit digit passes, query sort
+    nbatches = 3 if cfg["k"] else 2                             # query batches per step
+    pairs = totals["pairs"]
+    tree = 4 * (n * lw + (n - 1) * nw)                          # tree read once by a traversal
+    b = {
+        "B1_bounds": 4 * pw * n,
+        "B2_codes": 4 * pw * n + 8 * n,
+        "B3_sort_hist": 8 * n,
+        # pass 0 reads keys only (values are positions), later passes read and write (key,val)
+        "B3_sort_pass": (8 + 12) * n + (npass - 1) * 24 * n,
+        "B4_leaves": 4 * n + 4 * pw * n + 4 * lw * n,
+        # codes 8, leaf read, flag RMW 8, child box+ref write and read by the second arrival
+        "B5B6_hierarchy_refit": n * (8 + 4 * lw + 8) + (n - 1) * 2 * 4 * nw,
+        "Q1_qcodes": nbatches * 0,   # filled below per batch
+        "T2_scan": 4 * nq + 4 * nq + 4 * (nq + 1),
+    }
+    q1_spatial = 4 * qw * nq + 4 * nq
+    q1_knn = 4 * D * nq + 4 * nq
+    b["Q1_qcodes"] = 2 * q1_spatial + (q1_knn if cfg["k"] else 0)
+    b["Q2_qsort_hist"] = nbatches * 4 * nq
+    b["Q2_qsort_pass"] = nbatches * ((4 + 8) * nq + (qpass - 1) * 16 * nq)
+    # traversal: order 4 + query row + result; the tree is read once per traversal
+    per_count = nq * (4 + 4 * qw + 4) + tree
+    b["T1_spatial_count"] = 2 * per_count                       # once in _spatial, once in _count
+    b["T3_spatial_fill"] = nq * (4 + 4 * qw + 4) + 4 * pairs + tree
+    if cfg["k"]:
+        b["K1K2_knn"] = nq * (4 + 4 * D + 8 * cfg["k"]) + tree
+    return b
+
+
+def max_over_ranks(vals, device=None):
+    """MAX over all ranks of each entry of `vals` (identity without a process group)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in vals]
+    t = torch.tensor(list(vals), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def rank_seed_offset(rank: int) -> int:
+    """Replicas draw distinct inputs of the same law."""
+    return 1000 * rank
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.2] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1]))
+            except Exception:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(smax)) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---- the oracle, timed (cpu_baseline leg and --impl reference) ----------------------------------
+def oracle_step(cfg, sample: int):
+    """One bounded oracle 'step': grid build(s) over all N primitives + `sample` queries of each
+    batch kind.  Returns (seconds extrapolated to the full step, detail)."""
+    import oracle
+    prims, pk = cfg["prims"], cfg["pkind"]
+    nq = cfg["nq"]
+    s = min(sample, nq)
+    t0 = time.perf_counter()
+    grid = oracle.Grid(prims, pk, oracle.default_cell(prims, pk, "spatial", cfg["r"] if cfg["r"] else None))
+    t_build = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    off, _, _ = oracle.spatial(prims, pk, cfg["queries"][:s], cfg["qkind"], grid)
+    t_spatial = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    off2, _, _ = oracle.spatial(prims, pk, cfg["queries"][:s], cfg["qkind"], grid)   # count-only = same search
+    t_count = time.perf_counter() - t0
+    del grid
+    t_knn = t_kbuild = 0.0
+    if cfg["k"]:
+        t0 = time.perf_counter()
+        kgrid = oracle.Grid(prims, pk, oracle.default_cell(prims, pk, "knn"))
+        t_kbuild = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        oracle.knn(prims, pk, cfg["qpoints"][:s], cfg["k"], kgrid)
+        t_knn = time.perf_counter() - t0
+        del kgrid
+    nb = 3 if cfg["k"] else 2
+    full = t_build + t_kbuild + (nq / s) * (t_spatial + t_count + t_knn)
+    detail = dict(sample_queries_per_batch=s, t_grid_build_s=round(t_build + t_kbuild, 3),
+                  t_spatial_s=round(t_spatial, 3), t_count_s=round(t_count, 3), t_knn_s=round(t_knn, 3),
+                  build_mprims_s=round(cfg["n"] / max(t_build, 1e-9) / 1e6, 3),
+                  radius_qps=round(s / max(t_spatial, 1e-9), 1),
+                  knn_qps=round(s / t_knn, 1) if t_knn else None)
+    return full, nb * nq / full, detail
+
+
+def run_reference(args, cfg):
+    import oracle
+    oracle.build()
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cores = oracle.num_threads()
+    times, vals, detail = [], [], None
+    for i in range(args.warmup + args.steps):
+        full, v, detail = oracle_step(cfg, args.ref_sample)
+        if i >= args.warmup:
+            times.append(full); vals.append(v)
+    nb = 3 if cfg["k"] else 2
+    ms = 1e3 * float(np.mean(times))
+    value = nb * cfg["nq"] / (ms / 1e3)
+    sample = (f"per step: uniform-grid build over all {cfg['n']} primitives + first {detail['sample_queries_per_batch']} "
+              f"queries of each of the {nb} batches, query time extrapolated linearly to Q={cfg['nq']}")
+    line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic",
+                config=dict(workload=cfg["name"], n=cfg["n"], nq=cfg["nq"], dim=cfg["dim"], k=cfg["k"], r=cfg["r"]),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample, detail=detail),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink N and Q (debugging only; a scaled run is not a bench value)")
+    ap.add_argument("--ref-sample", type=int, default=200_000, help="oracle queries per batch per step")
+    ap.add_argument("--cpu-sample", type=int, default=500_000, help="cpu_baseline queries per batch")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print(f"note: --warmup {args.warmup} < 3 breaks the timing rules; use >= 3 for a reportable number", file=sys.stderr)
+
+    from paper_2507_23700_b200 import datagen as dg
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = dg.config(args.workload, args.scale, seed_offset=0 if args.impl == "reference" else rank_seed_offset(rank))
+
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2507_23700_b200 import binding as arbx
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    arbx.lib()   # fail loudly if the extension is missing
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    n, nq, D, k = cfg["n"], cfg["nq"], cfg["dim"], cfg["k"]
+    pk, qk = cfg["pkind"], cfg["qkind"]
+    stream = torch.cuda.Stream()
+    # pinned host inputs (e2e leg) and device-resident copies (value leg)
+    h_prims = torch.from_numpy(cfg["prims"]).pin_memory()
+    h_queries = torch.from_numpy(cfg["queries"]).pin_memory()
+    h_qpoints = torch.from_numpy(cfg["qpoints"]).pin_memory() if k else None
+    d_prims, d_queries = h_prims.to(dev), h_queries.to(dev)
+    d_qpoints = h_qpoints.to(dev) if k else None
+
+    # size the CSR buffer once (an untimed query: count + scan only)
+    with torch.cuda.stream(stream):
+        h0 = arbx.arbx_build(d_prims, D, pk, stream)
+        offsets = torch.empty(nq + 1, dtype=torch.int32, device=dev)
+        _, total = arbx.arbx_query_spatial(h0, d_queries, nq, qk, offsets, None, 0, stream)
+        arbx.arbx_destroy(h0, stream)
+    capacity = int(total)
+    indices = torch.empty(max(capacity, 1), dtype=torch.int32, device=dev)
+    counts = torch.empty(nq, dtype=torch.int32, device=dev)
+    kidx = torch.empty((nq, k), dtype=torch.int32, device=dev) if k else None
+    kdist = torch.empty((nq, k), dtype=torch.float32, device=dev) if k else None
+    nbatches = 3 if k else 2
+
+    marks = []   # (name, event) per step, on `stream`
+
+    def mark(name):
+        e = torch.cuda.Event(enable_timing=True)
+        e.record(stream)
+        marks.append((name, e))
+
+    def step(prims, queries, qpoints, timed_marks):
+        h = arbx.arbx_build(prims, D, pk, stream)
+        if timed_marks: mark("build")
+        arbx.arbx_query_spatial(h, queries, nq, qk, offsets, indices, capacity, stream)
+        if timed_marks: mark("spatial")
+        arbx.arbx_query_count(h, queries, nq, qk, counts, stream)
+        if timed_marks: mark("count")
+        if k:
+            arbx.arbx_query_knn(h, qpoints, nq, k, kidx, kdist, stream)
+            if timed_marks: mark("knn")
+        arbx.arbx_destroy(h, stream)
+
+    # ---- value leg: inputs resident in HBM --------------------------------------------------------
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            step(d_prims, d_queries, d_qpoints, False)
+        barrier()
+        sampler = ClockSampler(local_rank) if rank == 0 else None
+        arbx.arbx_profile_enable(True)
+        arbx.arbx_profile_read()
+        l0 = arbx.arbx_launch_count()
+        t_wall0 = time.time()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            mark("begin")
+            step(d_prims, d_queries, d_qpoints, True)
+        e1.record(stream)
+        barrier()
+        t_wall1 = time.time()
+        launches = arbx.arbx_launch_count() - l0
+        prof = arbx.arbx_profile_read()
+        arbx.arbx_profile_enable(False)
+        clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    ms_total = e0.elapsed_time(e1)
+    calls = {}
+    for (na, ea), (nb_, eb) in zip(marks[:-1], marks[1:]):
+        if nb_ != "begin":
+            calls[nb_] = calls.get(nb_, 0.0) + ea.elapsed_time(eb)
+    calls = {c: v / args.steps for c, v in calls.items()}
+    marks.clear()
+
+    # ---- e2e leg: pinned host inputs in, every result back to pinned host memory ---------------------
+    e2e = None
+    if not args.no_e2e:
+        ho = torch.empty(nq + 1, dtype=torch.int32).pin_memory()
+        hi = torch.empty(max(capacity, 1), dtype=torch.int32).pin_memory()
+        hc = torch.empty(nq, dtype=torch.int32).pin_memory()
+        hki = torch.empty((nq, k), dtype=torch.int32).pin_memory() if k else None
+        hkd = torch.empty((nq, k), dtype=torch.float32).pin_memory() if k else None
+        s_prims, s_queries = torch.empty_like(d_prims), torch.empty_like(d_queries)
+        s_qpoints = torch.empty_like(d_qpoints) if k else None
+
+        def e2e_step():
+            s_prims.copy_(h_prims, non_blocking=True)
+            s_queries.copy_(h_queries, non_blocking=True)
+            if k: s_qpoints.copy_(h_qpoints, non_blocking=True)
+            step(s_prims, s_queries, s_qpoints, False)
+            ho.copy_(offsets, non_blocking=True)
+            hi[:capacity].copy_(indices[:capacity], non_blocking=True)
+            hc.copy_(counts, non_blocking=True)
+            if k:
+                hki.copy_(kidx, non_blocking=True)
+                hkd.copy_(kdist, non_blocking=True)
+
+        with torch.cuda.stream(stream):
+            e2e_step()
+            barrier()
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(args.steps):
+                e2e_step()
+            b.record(stream)
+            barrier()
+        ms_e2e = a.elapsed_time(b) / args.steps
+        h2d = h_prims.numel() * 4 + h_queries.numel() * 4 + (h_qpoints.numel() * 4 if k else 0)
+        d2h = ho.numel() * 4 + capacity * 4 + hc.numel() * 4 + (hki.numel() * 8 if k else 0)
+        assert int(ho[-1]) == capacity and int(hc.sum()) == capacity, "e2e results inconsistent"
+    # max over ranks
+    ms_step = ms_total / args.steps
+    ms_step, ms_e2e_max = max_over_ranks([ms_step, ms_e2e if not args.no_e2e else 0.0], dev)
+    if not args.no_e2e:
+        e2e = dict(value=world * nbatches * nq / (ms_e2e_max / 1e3), unit=UNIT, ms_per_step=ms_e2e_max,
+                   h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h))
+
+    if rank == 0:
+        peak, peak_src = _peaks()
+        ab = algorithmic_bytes(cfg, dict(pairs=capacity))
+        kern = {}
+        for name, (ms, ncalls) in prof.items():
+            ms_s = ms / args.steps
+            by = ab.get(name)
+            kern[name] = dict(ms_per_step=round(ms_s, 4), launches_per_step=ncalls / args.steps,
+                              share=round(ms_s / ms_step, 4),
+                              algorithmic_gb=round(by / 1e9, 4) if by else None,
+                              achieved_gbs=round(by / 1e6 / ms_s, 1) if by and ms_s > 0 else None,
+                              frac_of_peak=round(by / 1e6 / ms_s / peak, 4) if by and ms_s > 0 else None)
+        dom = max(kern, key=lambda x: kern[x]["ms_per_step"])
+        dk = kern[dom]
+        # per-LAUNCH figures for the dominant kernel
+        lps = max(dk["launches_per_step"], 1)
+        roofline = dict(bound="hbm", kernel=dom, achieved=dk["achieved_gbs"], peak=peak, unit="GB/s",
+                        frac=dk["frac_of_peak"], traffic=None, peak_source=peak_src,
+                        algorithmic_bytes_per_launch=int(ab[dom] / lps) if ab.get(dom) else None,
+                        ms_per_launch=round(dk["ms_per_step"] / lps, 4), share_of_step=dk["share"])
+        build_bytes = sum(ab[x] for x in ab if x.startswith("B"))
+        breakdown = dict(
+            build_mprims_s=round(n / calls["build"] / 1e3, 2), build_ms=round(calls["build"], 4),
+            build_algorithmic_gbs=round(build_bytes / 1e6 / calls["build"], 1),
+            build_frac_of_peak=round(build_bytes / 1e6 / calls["build"] / peak, 4),
+            radius_csr_qps=round(nq / calls["spatial"] * 1e3, 1), radius_csr_ms=round(calls["spatial"], 4),
+            count_only_qps=round(nq / calls["count"] * 1e3, 1), count_only_ms=round(calls["count"], 4),
+            knn_qps=round(nq / calls["knn"] * 1e3, 1) if k else None, knn_ms=round(calls["knn"], 4) if k else None,
+            pairs=capacity, kernels=kern)
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            import oracle
+            oracle.build()
+            _, v, detail = oracle_step(cfg, args.cpu_sample)
+            cpu = dict(value=v, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                       sample=(f"uniform-grid build over all {n} primitives + first {detail['sample_queries_per_batch']} "
+                               f"queries of each of the {nbatches} batches of this workload, query time extrapolated linearly to Q={nq}"),
+                       detail=detail)
+        line = dict(metric=METRIC, value=world * nbatches * nq / (ms_step / 1e3), unit=UNIT, n_gpus=world,
+                    steps=args.steps, warmup=args.warmup, ms_per_step=ms_step, higher_is_better=True,
+                    scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                    config=dict(workload=cfg["name"], n=n, nq=nq, dim=D, k=k, r=cfg["r"], scale=args.scale,
+                                parallelism=f"replicas x{world}" if world > 1 else "single GPU",
+                                l2="inputs and outputs exceed L2 (no flush needed)" if (d_prims.numel() + d_queries.numel()) * 4 > 126e6 else "working set fits L2"),
+                    clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline,
+                    cpu_baseline=cpu, breakdown=breakdown)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

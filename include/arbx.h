@@ -136,6 +136,17 @@ ARBX_API arbx_status arbx_debug_validate(arbx_handle h, int64_t* violations_host
  * gpu_launches claim).                                                                      */
 ARBX_API int64_t arbx_launch_count(void);
 
+/* Per-step device timing, for the roofline figures of bench.py.  While
+ * enabled, every hot-path step (one entry of arbx_profile_kernel_name: "B3_sort_pass",
+ * "T1_spatial_count", "K1K2_knn", ...) is bracketed by a pair of CUDA events recorded on the
+ * stream it is launched on.  arbx_profile_read waits for the recorded events, adds up the
+ * elapsed milliseconds and the number of bracketed steps per kernel id into the HOST arrays
+ * ms_host / calls_host (capacity >= arbx_profile_num_kernels()) and clears the record.      */
+ARBX_API arbx_status arbx_profile_enable(int on);
+ARBX_API int arbx_profile_num_kernels(void);
+ARBX_API const char* arbx_profile_kernel_name(int id);
+ARBX_API arbx_status arbx_profile_read(double* ms_host, int64_t* calls_host, int capacity);
+
 ARBX_API const char* arbx_status_string(arbx_status s);
 ARBX_API const char* arbx_last_error(void);          /* thread-local detail of the last failure */
 

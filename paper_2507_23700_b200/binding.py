@@ -24,7 +24,8 @@ LIB_PATH = os.path.join(_HERE, "libarbx.so")
 EXPORTS = (
     "arbx_build", "arbx_destroy", "arbx_size", "arbx_bounds", "arbx_query_count",
     "arbx_query_spatial", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
-    "arbx_launch_count", "arbx_status_string", "arbx_last_error",
+    "arbx_launch_count", "arbx_profile_enable", "arbx_profile_num_kernels",
+    "arbx_profile_kernel_name", "arbx_profile_read", "arbx_status_string", "arbx_last_error",
 )
 
 
@@ -58,6 +59,13 @@ def lib() -> ctypes.CDLL:
         L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
         L.arbx_debug_validate.argtypes = [vp, ctypes.POINTER(i64), vp]
         L.arbx_launch_count.restype = i64
+        L.arbx_profile_enable.argtypes = [i32]
+        L.arbx_profile_enable.restype = i32
+        L.arbx_profile_num_kernels.restype = i32
+        L.arbx_profile_kernel_name.argtypes = [i32]
+        L.arbx_profile_kernel_name.restype = ctypes.c_char_p
+        L.arbx_profile_read.argtypes = [vp, vp, i32]
+        L.arbx_profile_read.restype = i32
         L.arbx_status_string.restype = ctypes.c_char_p
         L.arbx_status_string.argtypes = [i32]
         L.arbx_last_error.restype = ctypes.c_char_p
@@ -159,6 +167,20 @@ def arbx_debug_validate(handle: int, stream=None) -> int:
 
 def arbx_launch_count() -> int:
     return int(lib().arbx_launch_count())
+
+
+def arbx_profile_enable(on: bool) -> None:
+    _check(lib().arbx_profile_enable(1 if on else 0), "arbx_profile_enable")
+
+
+def arbx_profile_read() -> dict:
+    """{kernel name: (milliseconds, bracketed steps)} accumulated since the last read."""
+    L = lib()
+    nk = L.arbx_profile_num_kernels()
+    ms = (ctypes.c_double * nk)()
+    calls = (ctypes.c_int64 * nk)()
+    _check(L.arbx_profile_read(ctypes.addressof(ms), ctypes.addressof(calls), nk), "arbx_profile_read")
+    return {L.arbx_profile_kernel_name(i).decode(): (ms[i], calls[i]) for i in range(nk) if calls[i]}
 
 
 # ---- convenience wrapper -----------------------------------------------------------------------

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <mutex>
+#include <vector>
 
 #include "common.cuh"
 
@@ -22,6 +23,41 @@ void set_error(const char* fmt, ...) {
   va_start(ap, fmt);
   vsnprintf(t_err, sizeof(t_err), fmt, ap);
   va_end(ap);
+}
+
+// ---- per-kernel timing ---------------------------------------------------------------------
+static std::atomic<int> g_prof_on{0};
+static std::mutex g_prof_mu;
+struct ProfRec { int id; cudaEvent_t a, b; };
+static std::vector<ProfRec> g_prof_open, g_prof_done;
+static std::vector<cudaEvent_t> g_prof_pool;
+static const char* const kKernelNames[K_NUM_] = {
+    "B1_bounds", "B2_codes", "B3_sort_hist", "B3_sort_pass", "B4_leaves", "B5B6_hierarchy_refit",
+    "Q1_qcodes", "Q2_qsort_hist", "Q2_qsort_pass", "T1_spatial_count", "T2_scan", "T3_spatial_fill",
+    "K1K2_knn", "misc"};
+
+bool prof_enabled() { return g_prof_on.load(std::memory_order_relaxed) != 0; }
+static cudaEvent_t prof_event() {
+  if (!g_prof_pool.empty()) { cudaEvent_t e = g_prof_pool.back(); g_prof_pool.pop_back(); return e; }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+void prof_begin(int id, cudaStream_t s) {
+  std::lock_guard<std::mutex> g(g_prof_mu);
+  ProfRec r{id, prof_event(), prof_event()};
+  cudaEventRecord(r.a, s);
+  g_prof_open.push_back(r);
+}
+void prof_end(int id, cudaStream_t s) {
+  std::lock_guard<std::mutex> g(g_prof_mu);
+  for (size_t i = g_prof_open.size(); i-- > 0;)
+    if (g_prof_open[i].id == id) {
+      cudaEventRecord(g_prof_open[i].b, s);
+      g_prof_done.push_back(g_prof_open[i]);
+      g_prof_open.erase(g_prof_open.begin() + i);
+      return;
+    }
 }
 
 static std::once_flag g_pool_once[64];
@@ -246,6 +282,37 @@ arbx_status arbx_debug_validate(arbx_handle h, int64_t* violations_host, arbx_st
 }
 
 int64_t arbx_launch_count(void) { return (int64_t)g_launches.load(); }
+
+arbx_status arbx_profile_enable(int on) {
+  g_prof_on.store(on ? 1 : 0);
+  return ARBX_OK;
+}
+
+int arbx_profile_num_kernels(void) { return K_NUM_; }
+
+const char* arbx_profile_kernel_name(int id) { return id >= 0 && id < K_NUM_ ? kKernelNames[id] : ""; }
+
+arbx_status arbx_profile_read(double* ms_host, int64_t* calls_host, int capacity) {
+  if (!ms_host || !calls_host || capacity < K_NUM_) {
+    set_error("arbx_profile_read: need capacity >= %d", (int)K_NUM_);
+    return ARBX_ERR_INVALID_ARG;
+  }
+  for (int i = 0; i < capacity; ++i) { ms_host[i] = 0.0; calls_host[i] = 0; }
+  std::lock_guard<std::mutex> g(g_prof_mu);
+  arbx_status st = ARBX_OK;
+  for (const ProfRec& r : g_prof_done) {
+    float ms = 0.f;
+    cudaError_t e = cudaEventSynchronize(r.b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.a, r.b);
+    if (e != cudaSuccess) { set_error("arbx_profile_read: %s", cudaGetErrorString(e)); st = ARBX_ERR_CUDA; }
+    ms_host[r.id] += ms;
+    calls_host[r.id] += 1;
+    g_prof_pool.push_back(r.a);
+    g_prof_pool.push_back(r.b);
+  }
+  g_prof_done.clear();
+  return st;
+}
 
 const char* arbx_status_string(arbx_status s) {
   switch (s) {

@@ -200,28 +200,38 @@ arbx_status build_typed(const float* prims, int64_t n, cudaStream_t s, Index* ix
   Scratch<uint32_t> enc, perm;
   Scratch<int> flags;
   ARBX_TRY(enc.alloc(2 * D, s));
-  bounds_init_kernel<<<1, 32, 0, s>>>(enc.p, D);
-  ARBX_LAUNCH_CHECK();
   const int sgrid = grid_for(n, BT, sms * 8);
-  bounds_kernel<D, PK><<<sgrid, BT, 0, s>>>(prims, n, enc.p);
-  ARBX_LAUNCH_CHECK();
-  bounds_decode_kernel<<<1, 32, 0, s>>>(enc.p, ix->bounds, D);
-  ARBX_LAUNCH_CHECK();
+  {
+    ProfScope ps(K_BOUNDS, s);
+    bounds_init_kernel<<<1, 32, 0, s>>>(enc.p, D);
+    ARBX_LAUNCH_CHECK();
+    bounds_kernel<D, PK><<<sgrid, BT, 0, s>>>(prims, n, enc.p);
+    ARBX_LAUNCH_CHECK();
+    bounds_decode_kernel<<<1, 32, 0, s>>>(enc.p, ix->bounds, D);
+    ARBX_LAUNCH_CHECK();
+  }
 
   ARBX_TRY(scratch_alloc((void**)&ix->codes, (size_t)n * sizeof(unsigned long long), s));
-  codes_kernel<D, PK><<<sgrid, BT, 0, s>>>(prims, n, ix->bounds, ix->codes);
-  ARBX_LAUNCH_CHECK();
+  {
+    ProfScope ps(K_CODES, s);
+    codes_kernel<D, PK><<<sgrid, BT, 0, s>>>(prims, n, ix->bounds, ix->codes);
+    ARBX_LAUNCH_CHECK();
+  }
   ARBX_TRY(perm.alloc((size_t)n, s));
   ARBX_TRY(radix_sort_u64(ix->codes, perm.p, true, n, D * code_bits_per_axis(D), s));
 
   ARBX_TRY(scratch_alloc((void**)&ix->leaves, (size_t)n * LW * sizeof(float), s));
   const int fgrid = (int)((n + BT - 1) / BT);
-  leaves_kernel<D, PK><<<fgrid, BT, 0, s>>>(prims, perm.p, n, ix->leaves);
-  ARBX_LAUNCH_CHECK();
+  {
+    ProfScope ps(K_LEAVES, s);
+    leaves_kernel<D, PK><<<fgrid, BT, 0, s>>>(prims, perm.p, n, ix->leaves);
+    ARBX_LAUNCH_CHECK();
+  }
 
   const size_t nn = n > 1 ? (size_t)(n - 1) : 1;
   ARBX_TRY(scratch_alloc((void**)&ix->nodes, nn * NW * sizeof(float), s));
   ARBX_TRY(flags.alloc(nn, s));
+  ProfScope ps(K_HIERARCHY, s);
   ARBX_CUDA(cudaMemsetAsync(flags.p, 0xff, nn * sizeof(int), s));
   hierarchy_kernel<D, PK><<<fgrid, BT, 0, s>>>(ix->codes, ix->leaves, ix->nodes, flags.p, (int)n,
                                                ix->leaf_max, ix->root);

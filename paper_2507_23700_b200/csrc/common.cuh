@@ -61,6 +61,20 @@ inline void count_launch(int k = 1) { g_launches.fetch_add(k, std::memory_order_
     }                                                                                    \
   } while (0)
 
+// ---- per-kernel timing (arbx_profile_*): CUDA events on the launching stream ---------------
+enum KernelId {
+  K_BOUNDS = 0, K_CODES, K_SORT_HIST, K_SORT_PASS, K_LEAVES, K_HIERARCHY, K_QCODE, K_QSORT_HIST,
+  K_QSORT_PASS, K_SPATIAL_COUNT, K_SCAN, K_SPATIAL_FILL, K_KNN, K_MISC, K_NUM_
+};
+bool prof_enabled();
+void prof_begin(int id, cudaStream_t s);
+void prof_end(int id, cudaStream_t s);
+struct ProfScope {   // brackets the launches of one hot-path step with a pair of events
+  int id; cudaStream_t s; bool on;
+  ProfScope(int id_, cudaStream_t s_) : id(id_), s(s_), on(prof_enabled()) { if (on) prof_begin(id, s); }
+  ~ProfScope() { if (on) prof_end(id, s); }
+};
+
 #define ARBX_LAUNCH_CHECK()                                                              \
   do {                                                                                   \
     ::arbx::count_launch();                                                              \

@@ -349,6 +349,7 @@ arbx_status spatial_launch(const Index* ix, const float* queries, int64_t nq, co
   const unsigned grid = (unsigned)((nq + QT - 1) / QT);
   const float4* nodes = reinterpret_cast<const float4*>(ix->nodes);
   const float4* leaves = reinterpret_cast<const float4*>(ix->leaves);
+  ProfScope ps(indices ? K_SPATIAL_FILL : K_SPATIAL_COUNT, s);
   if (indices)
     spatial_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
   else
@@ -380,6 +381,7 @@ template <int PK, class Heap>
 arbx_status knn_launch(const Index* ix, const float* qpoints, int64_t nq, int k, const uint32_t* qorder,
                        int32_t* indices, float* distances, cudaStream_t s) {
   const unsigned grid = (unsigned)((nq + QT - 1) / QT);
+  ProfScope ps(K_KNN, s);
   knn_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
                                            reinterpret_cast<const float4*>(ix->leaves), ix->root, qpoints,
                                            qorder, nq, k, ix->n, indices, distances);
@@ -414,6 +416,7 @@ arbx_status qcode_entry(const Index* ix, const float* queries, int64_t nq, int q
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((nq + 255) / 256, (int64_t)sms * 8));
+  ProfScope ps(K_QCODE, s);
   switch (qkind) {
     case KIND_POINT: qcode_kernel<KIND_POINT><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes); break;
     case KIND_BOX: qcode_kernel<KIND_BOX><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes); break;

@@ -87,6 +87,7 @@ arbx_status exclusive_scan_i32(const int32_t* counts, int32_t* offsets, int64_t 
     return ARBX_OK;
   }
   const int nb = (int)((nq + SB - 1) / SB);
+  ProfScope ps(K_SCAN, s);
   Scratch<long long> sums;
   ARBX_TRY(sums.alloc(nb, s));
   block_sums_kernel<<<nb, ST, 0, s>>>(counts, nq, sums.p);

@@ -241,7 +241,10 @@ arbx_status radix_sort_impl(K* keys, uint32_t* vals, bool iota, int64_t n, int k
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  constexpr int kHistId = sizeof(K) == 8 ? K_SORT_HIST : K_QSORT_HIST;
+  constexpr int kPassId = sizeof(K) == 8 ? K_SORT_PASS : K_QSORT_PASS;
   {
+    ProfScope ps(kHistId, s);
     int64_t want = (n / (16 / (int)sizeof(K)) + 511) / 512;
     int grid = (int)std::min<int64_t>(std::max<int64_t>(want, 1), (int64_t)sms * 4);
     hist_kernel<K><<<grid, 512, 0, s>>>(keys, (uint32_t)n, npass, ghist);
@@ -254,6 +257,7 @@ arbx_status radix_sort_impl(K* keys, uint32_t* vals, bool iota, int64_t n, int k
   for (int p = 0; p < npass; ++p) {
     const uint32_t* base = ghist + (size_t)p * RADIX;
     uint32_t* st = status + (size_t)p * ntiles * RADIX;
+    ProfScope ps(kPassId, s);
     if (!has_vals)
       onesweep_pass<K, false, false><<<ntiles, SORT_THREADS, 0, s>>>(kin, kout, nullptr, nullptr, (uint32_t)n, 8 * p, base, counters + p, st);
     else if (p == 0 && iota)

@@ -88,32 +88,35 @@ def gaussian_mixture(n: int, dim: int, seed: int, centre_seed: int = 2, ncomp: i
 CONFIG_NAMES = ("C1", "C2", "C3", "C4", "C5")
 
 
-def config(name: str, scale: float = 1.0) -> dict:
+def config(name: str, scale: float = 1.0, seed_offset: int = 0) -> dict:
     """The five BASELINE.json workloads. `scale` < 1 shrinks N and Q (same law, same density
     relations) for quick parity cases; scale == 1 is the size BASELINE.json states.
+    `seed_offset` shifts the data/query seeds (0, 1) so that bench.py replicas draw distinct
+    inputs of the same law; the parity tests always use offset 0.
 
     Returns dict(prims, pkind, dim, queries (spatial layout), qkind, qpoints (kNN) or None,
                  k or None, r or None, name, n, nq).
     """
+    s0, s1 = seed_offset, seed_offset + 1
     if name == "C1":
         n = nq = max(1, int(10_000 * scale))
-        p = uniform_points(n, 3, 0)
-        qp = uniform_points(nq, 3, 1)
+        p = uniform_points(n, 3, s0)
+        qp = uniform_points(nq, 3, s1)
         r = 0.0620
         return dict(name=name, prims=p, pkind=POINT, dim=3, queries=sphere_queries(qp, r),
                     qkind=SPHERE, qpoints=qp, k=10, r=r, n=n, nq=nq)
     if name == "C2":
         n = nq = max(1, int(1_000_000 * scale))
-        p = uniform_points(n, 3, 0)
-        qp = uniform_points(nq, 3, 1)
+        p = uniform_points(n, 3, s0)
+        qp = uniform_points(nq, 3, s1)
         r = radius_for_expected(16.0, float(n), 3)
         return dict(name=name, prims=p, pkind=POINT, dim=3, queries=sphere_queries(qp, r),
                     qkind=SPHERE, qpoints=qp, k=None, r=r, n=n, nq=nq)
     if name == "C3":
         n = nq = max(1, int(10_000_000 * scale))
         a = float(n) ** (1.0 / 3.0)
-        p = uniform_points(n, 3, 0, scale=a)
-        g = rng(1)
+        p = uniform_points(n, 3, s0, scale=a)
+        g = rng(s1)
         v = g.standard_normal((nq, 3))
         v /= np.linalg.norm(v, axis=1, keepdims=True)
         qp = (0.5 * a + 0.5 * a * v).astype(np.float32)
@@ -124,15 +127,15 @@ def config(name: str, scale: float = 1.0) -> dict:
         n = max(1, int(10_000_000 * scale))
         nq = max(1, int(5_000_000 * scale))
         h = 0.5 * float(n) ** (-1.0 / 3.0)
-        p = uniform_boxes(n, 3, 0, h)
-        q = uniform_boxes(nq, 3, 1, 2.0 * h)
+        p = uniform_boxes(n, 3, s0, h)
+        q = uniform_boxes(nq, 3, s1, 2.0 * h)
         return dict(name=name, prims=p, pkind=BOX, dim=3, queries=q, qkind=BOX,
                     qpoints=None, k=None, r=None, n=n, nq=nq)
     if name == "C5":
         n = max(1, int(4_000_000 * scale))
         nq = max(1, int(1_000_000 * scale))
-        p = gaussian_mixture(n, 5, 0)
-        qp = gaussian_mixture(nq, 5, 1)
+        p = gaussian_mixture(n, 5, s0)
+        qp = gaussian_mixture(nq, 5, s1)
         r = 0.01
         return dict(name=name, prims=p, pkind=POINT, dim=5, queries=sphere_queries(qp, r),
                     qkind=SPHERE, qpoints=qp, k=8, r=r, n=n, nq=nq)
