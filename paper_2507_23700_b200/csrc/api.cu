@@ -152,7 +152,7 @@ arbx_status arbx_build(const float* prims, int64_t n, int dim, arbx_kind kind, a
   if (n > kMaxCount) { set_error("arbx_build: n > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
   cudaStream_t s = (cudaStream_t)stream;
   arbx_index_s* h = new arbx_index_s();
-  h->ix.leaf_max = std::max(1, std::min(64, env_int("ARBX_LEAF_MAX", 4)));
+  h->ix.leaf_max = std::max(1, std::min(64, env_int("ARBX_LEAF_MAX", 16)));
   arbx_status st = build_index(prims, n, dim, (int)kind, s, &h->ix);
   if (st != ARBX_OK) {
     free_index(&h->ix, s);

@@ -115,29 +115,81 @@ __global__ void __launch_bounds__(BT) leaves_kernel(const float* __restrict__ pr
 }
 
 // ---- B5+B6: bottom-up hierarchy with fused refit ------------------------------------------------
-// Adjacent-leaf metric: XOR of the two codes; equal codes fall back to the XOR of the sorted
-// positions (SURVEY.md reading A16), ordered below every non-zero code XOR.
-struct Delta { unsigned long long x; uint32_t ix; };
-__device__ __forceinline__ Delta delta_at(const unsigned long long* __restrict__ codes, int i) {
-  Delta d;
-  d.x = __ldg(codes + i) ^ __ldg(codes + i + 1);
-  d.ix = (uint32_t)i ^ (uint32_t)(i + 1);
-  return d;
+// The tree is the binary radix tree of the sorted codes (Karras 2012): internal node p sits at
+// the split between sorted leaves p and p+1, and a subtree covering [l,r] hangs under split r
+// or split l-1, whichever separates codes that share the LONGER prefix.  Only the position of
+// the highest differing bit matters for that comparison (two splits with the same highest bit
+// always have a higher one between them, so they never bound the same range), so every split j
+// is reduced to one byte:
+//   level(j) = 32 + (1 + index of the top set bit of code[j]^code[j+1])      distinct codes
+//            =      (1 + index of the top set bit of j^(j+1))                equal codes (A16:
+//              duplicates are split by sorted position, which yields a balanced subtree)
+//            = 255  for j = -1 and j = n-1 (the ends of the array).
+// Emission is bottom-up (Apetrei 2014): every leaf climbs; at each node the first
+// child to arrive leaves its box and stops, the second merges both boxes and carries on.
+// B200 design: a block owns a chunk of HB consecutive leaves and does every merge whose node
+// range lies inside the chunk through SHARED memory (flag + sibling box, __threadfence_block
+// only).  A node is chunk-local iff its level is below the running maximum on both sides inside
+// the chunk (prefix / suffix maxima of the level bytes), a property both children evaluate
+// identically.  Only the O(log HB) subtrees per chunk that stick out continue through global
+// atomics + __threadfence, so the long dependent chain of global round trips disappears.
+template <int D> struct HierCfg { static constexpr int HB = D <= 5 ? 512 : 256; };
+
+__device__ __forceinline__ int split_level(const unsigned long long* __restrict__ codes, int j, int n) {
+  if (j < 0 || j >= n - 1) return 255;
+  const unsigned long long x = __ldg(codes + j) ^ __ldg(codes + j + 1);
+  return x ? 32 + 64 - __clzll((long long)x) : 32 - __clz(j ^ (j + 1));
 }
-__device__ __forceinline__ bool delta_less(const Delta& a, const Delta& b) {
-  return a.x != b.x ? a.x < b.x : a.ix < b.ix;
+
+// inclusive running maximum over the block, thread order
+template <int HB>
+__device__ __forceinline__ int block_running_max(int v, int* s_w) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(~0u, v, o);
+    if (lane >= o) v = max(v, y);
+  }
+  if (lane == 31) s_w[w] = v;
+  __syncthreads();
+  int base = 0;
+  for (int i = 0; i < w; ++i) base = max(base, s_w[i]);
+  __syncthreads();
+  return max(v, base);
 }
 
 template <int D, int PK>
-__global__ void __launch_bounds__(BT) hierarchy_kernel(const unsigned long long* __restrict__ codes,
-                                                       float* __restrict__ leaves, float* __restrict__ nodes,
-                                                       int* __restrict__ flags, int n, int leaf_max,
-                                                       int32_t* __restrict__ root) {
+__global__ void __launch_bounds__(HierCfg<D>::HB)
+hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict__ leaves,
+                 float* __restrict__ nodes, int* __restrict__ flags, int n, int leaf_max,
+                 int32_t* __restrict__ root) {
+  constexpr int HB = HierCfg<D>::HB;
   constexpr int W = prim_width(PK, D);
   constexpr int LW = leaf_width(PK, D);
   constexpr int NW = node_width(D);
-  const int i = blockIdx.x * BT + threadIdx.x;
+  // s_lvl[t] = level of split c0-1+t, t = 0..HB;  s_pre[t] = max s_lvl[0..t];  s_suf[t] = max s_lvl[t..HB]
+  __shared__ uint8_t s_lvl[HB + 1], s_pre[HB + 1], s_suf[HB + 1];
+  __shared__ int s_w[HB / 32];
+  __shared__ int s_flag[HB];
+  __shared__ float s_box[2][HB][2 * D];
+  const int tid = threadIdx.x;
+  const int c0 = blockIdx.x * HB;
+  const int i = c0 + tid;
+  {
+    const int lv = split_level(codes, c0 - 1 + tid, n);
+    s_lvl[tid] = (uint8_t)lv;
+    s_flag[tid] = -1;
+    const int pm = block_running_max<HB>(lv, s_w);
+    s_pre[tid] = (uint8_t)pm;
+    // suffix maxima: thread t handles element HB - t (elements HB..1)
+    const int lr = split_level(codes, c0 - 1 + HB - tid, n);
+    if (tid == 0) s_lvl[HB] = (uint8_t)lr;
+    const int sm = block_running_max<HB>(lr, s_w);
+    s_suf[HB - tid] = (uint8_t)sm;
+  }
+  __syncthreads();
   if (i >= n) return;
+
   int l = i, r = i;
   int32_t ref = ~i;
   float lo[D], hi[D];
@@ -156,30 +208,47 @@ __global__ void __launch_bounds__(BT) hierarchy_kernel(const unsigned long long*
       return;
     }
     // the parent splits either right after r (we are its left child) or right before l
-    bool left_child;
-    if (l == 0) left_child = true;
-    else if (r == n - 1) left_child = false;
-    else left_child = delta_less(delta_at(codes, r), delta_at(codes, l - 1));
+    const bool inside = l >= c0 && r < c0 + HB;     // still chunk-local: levels come from shared memory
+    const int lvl_l = inside ? s_lvl[l - c0] : split_level(codes, l - 1, n);
+    const int lvl_r = inside ? s_lvl[r - c0 + 1] : split_level(codes, r, n);
+    const bool left_child = lvl_r < lvl_l;
     const int p = left_child ? r : l - 1;
+    const int t = p - c0 + 1;                        // index of split p in s_lvl
+    const bool local = inside && t >= 1 && t <= HB - 1 &&
+                       (left_child ? s_lvl[t] < s_suf[t + 1] : s_lvl[t] < s_pre[t - 1]);
     float* node = nodes + (int64_t)p * NW;
     const int slot = left_child ? 0 : 1;
+    const int sib = 1 - slot;
 #pragma unroll
     for (int a = 0; a < D; ++a) {
       __stcg(node + slot * 2 * D + a, lo[a]);
       __stcg(node + slot * 2 * D + D + a, hi[a]);
     }
     __stcg(reinterpret_cast<int*>(node) + 4 * D + slot, ref);
-    __threadfence();
-    const int other = atomicExch(flags + p, left_child ? l : r);
-    if (other == -1) return;     // first to arrive: the sibling's thread carries on
-    __threadfence();
-    // second to arrive: `other` is the far end of the sibling's range
-    const int sib = 1 - slot;
+    int other;
+    if (local) {
+      float* mine = s_box[slot][p - c0];
 #pragma unroll
-    for (int a = 0; a < D; ++a) {
-      lo[a] = fminf(lo[a], __ldcg(node + sib * 2 * D + a));
-      hi[a] = fmaxf(hi[a], __ldcg(node + sib * 2 * D + D + a));
+      for (int a = 0; a < D; ++a) { mine[a] = lo[a]; mine[D + a] = hi[a]; }
+      __threadfence_block();
+      other = atomicExch(&s_flag[p - c0], left_child ? l : r);
+      if (other == -1) return;   // first to arrive: the sibling's thread carries on
+      __threadfence_block();
+      const volatile float* theirs = s_box[sib][p - c0];
+#pragma unroll
+      for (int a = 0; a < D; ++a) { lo[a] = fminf(lo[a], theirs[a]); hi[a] = fmaxf(hi[a], theirs[D + a]); }
+    } else {
+      __threadfence();
+      other = atomicExch(flags + p, left_child ? l : r);
+      if (other == -1) return;
+      __threadfence();
+#pragma unroll
+      for (int a = 0; a < D; ++a) {
+        lo[a] = fminf(lo[a], __ldcg(node + sib * 2 * D + a));
+        hi[a] = fmaxf(hi[a], __ldcg(node + sib * 2 * D + D + a));
+      }
     }
+    // second to arrive: `other` is the far end of the sibling's range
     if (left_child) r = other; else l = other;
     __stcg(reinterpret_cast<int*>(node) + 4 * D + 2, l);
     __stcg(reinterpret_cast<int*>(node) + 4 * D + 3, r);
@@ -233,8 +302,9 @@ arbx_status build_typed(const float* prims, int64_t n, cudaStream_t s, Index* ix
   ARBX_TRY(flags.alloc(nn, s));
   ProfScope ps(K_HIERARCHY, s);
   ARBX_CUDA(cudaMemsetAsync(flags.p, 0xff, nn * sizeof(int), s));
-  hierarchy_kernel<D, PK><<<fgrid, BT, 0, s>>>(ix->codes, ix->leaves, ix->nodes, flags.p, (int)n,
-                                               ix->leaf_max, ix->root);
+  constexpr int HB = HierCfg<D>::HB;
+  hierarchy_kernel<D, PK><<<(unsigned)((n + HB - 1) / HB), HB, 0, s>>>(ix->codes, ix->leaves, ix->nodes, flags.p,
+                                                                      (int)n, ix->leaf_max, ix->root);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }

@@ -45,20 +45,6 @@ __global__ void __launch_bounds__(256) qcode_kernel(const float* __restrict__ qu
 }
 
 // ---- node / leaf access ------------------------------------------------------------------------
-struct Node { float v[4 * D]; int32_t c0, c1; };
-
-__device__ __forceinline__ void load_node(const float4* __restrict__ nodes, int32_t ref, Node& nd) {
-  const float4* p = nodes + (int64_t)ref * (D + 1);
-#pragma unroll
-  for (int e = 0; e < D; ++e) {
-    float4 t = __ldg(p + e);
-    nd.v[4 * e] = t.x; nd.v[4 * e + 1] = t.y; nd.v[4 * e + 2] = t.z; nd.v[4 * e + 3] = t.w;
-  }
-  float4 t = __ldg(p + D);
-  nd.c0 = __float_as_int(t.x);
-  nd.c1 = __float_as_int(t.y);
-}
-
 template <int PK>
 struct Leaf { float v[prim_width(PK, D)]; uint32_t idx; };
 
@@ -134,63 +120,116 @@ __device__ __forceinline__ bool hits_prim(const Query<QK>& q, const float* p) {
 }
 
 // ---- T1 / T3: spatial traversal ------------------------------------------------------------------
+// Warp-cooperative ("packet") traversal.  A warp owns 32 queries that are neighbours on the
+// space-filling curve and walks the tree ONCE for all of them: every lane tests its own query
+// against the two child boxes of the current node, the warp descends where ANY lane hits.
+// All lanes fetch the same node / leaf record, so a fetch is one broadcast L1 transaction
+// instead of 32 divergent ones, control flow is uniform, and the stack is one short array
+// per warp in shared memory.  The leaf test is per lane and exact, so the result is the same
+// set as one-query-per-thread traversal.
+struct NodeX { float v[4 * D]; int32_t c0, c1, l, r; };
+
+__device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, int32_t ref, NodeX& nd) {
+  const float4* p = nodes + (int64_t)ref * (D + 1);
+#pragma unroll
+  for (int e = 0; e < D; ++e) {
+    float4 t = __ldg(p + e);
+    nd.v[4 * e] = t.x; nd.v[4 * e + 1] = t.y; nd.v[4 * e + 2] = t.z; nd.v[4 * e + 3] = t.w;
+  }
+  float4 t = __ldg(p + D);
+  nd.c0 = __float_as_int(t.x); nd.c1 = __float_as_int(t.y);
+  nd.l = __float_as_int(t.z); nd.r = __float_as_int(t.w);
+}
+
 template <int PK, int QK, bool FILL>
 __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ nodes,
                                                      const float4* __restrict__ leaves,
-                                                     const int32_t* __restrict__ root,
+                                                     const int32_t* __restrict__ root, int n,
                                                      const float* __restrict__ queries,
                                                      const uint32_t* __restrict__ qorder, int64_t nq,
                                                      int32_t* __restrict__ counts,
                                                      const int32_t* __restrict__ offsets,
                                                      int32_t* __restrict__ indices) {
   constexpr int QW = prim_width(QK, D);
+  __shared__ int32_t s_stack[QT / 32][STACK_DEPTH];
+  int32_t* stack = s_stack[threadIdx.x >> 5];
   const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
-  if (t >= nq) return;
-  const int64_t qi = qorder ? (int64_t)qorder[t] : t;
+  const bool valid = t < nq;
+  const int64_t qi = valid ? (qorder ? (int64_t)qorder[t] : t) : 0;
   Query<QK> q;
 #pragma unroll
   for (int e = 0; e < QW; ++e) q.v[e] = __ldg(queries + qi * QW + e);
-  bool alive = true;
+  bool alive = valid;
   if constexpr (QK == KIND_SPHERE) {
     q.r2 = q.v[D] * q.v[D];
-    alive = q.v[D] >= 0.f;      // negative radius matches nothing (reading A21)
+    alive = alive && q.v[D] >= 0.f;      // negative radius matches nothing (reading A21)
   }
-  int32_t* out = nullptr;
-  if constexpr (FILL) out = indices + offsets[qi];
-  int cnt = 0;
-  if (alive) {
-    int32_t stack[STACK_DEPTH];
-    int sp = 0;
-    int32_t ref = __ldg(root);
-    for (;;) {
-      if (ref >= 0) {
-        Node nd;
-        load_node(nodes, ref, nd);
-        const bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
-        const bool h1 = hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D);
-        if (h0) {
-          ref = nd.c0;
-          if (h1) stack[sp++] = nd.c1;
-          continue;
-        }
-        if (h1) { ref = nd.c1; continue; }
+  // FILL: hits are staged per lane in shared memory (FS slots, column `lane` of a padded
+  // [FS][33] array) and flushed row by row with all lanes writing one query's pending hits as
+  // one contiguous run, instead of one scattered 4-byte store per hit.
+  constexpr int FS = 16;
+  __shared__ int32_t s_stage[FILL ? QT / 32 : 1][FILL ? FS * 33 : 1];
+  int32_t* stage = s_stage[FILL ? (threadIdx.x >> 5) : 0];
+  const int lane = threadIdx.x & 31;
+  int base = 0;      // FILL: position in `indices` of this query's next unflushed hit
+  if constexpr (FILL) base = valid ? offsets[qi] : 0;
+  int cnt = 0, pend = 0;
+
+  auto flush = [&]() {
+    __syncwarp();
+    for (int L = 0; L < 32; ++L) {
+      const int m = __shfl_sync(~0u, pend, L);
+      const int b = __shfl_sync(~0u, base, L);
+      if (lane < m) indices[b + lane] = stage[lane * 33 + L];
+    }
+    base += pend;
+    pend = 0;
+    __syncwarp();
+  };
+
+  auto leaf_range = [&](int first, int m) {   // m is warp-uniform
+#pragma unroll 4
+    for (int j = 0; j < m; ++j) {
+      Leaf<PK> lf;
+      load_leaf<PK>(leaves, first + j, lf);
+      const bool hit = alive && hits_prim<QK, PK>(q, lf.v);
+      if constexpr (FILL) {
+        if (hit) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
+        if (__any_sync(~0u, pend == FS)) flush();
       } else {
-        int j = ~ref;
-        for (;; ++j) {
-          Leaf<PK> lf;
-          load_leaf<PK>(leaves, j, lf);
-          if (hits_prim<QK, PK>(q, lf.v)) {
-            if constexpr (FILL) out[cnt] = (int32_t)(lf.idx & ~LEAF_END);
-            ++cnt;
-          }
-          if (lf.idx & LEAF_END) break;
+        cnt += hit ? 1 : 0;
+      }
+    }
+  };
+
+  if (__any_sync(~0u, alive)) {
+    int32_t ref = __ldg(root);
+    if (ref < 0) {
+      leaf_range(0, n);
+    } else {
+      int sp = 0;
+      for (;;) {
+        NodeX nd;
+        load_node_x(nodes, ref, nd);
+        const bool a0 = __any_sync(~0u, alive && hits_box<QK>(q, nd.v, nd.v + D));
+        const bool a1 = __any_sync(~0u, alive && hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D));
+        if (a0 && nd.c0 < 0) leaf_range(nd.l, ref - nd.l + 1);
+        if (a1 && nd.c1 < 0) leaf_range(ref + 1, nd.r - ref);
+        const bool in0 = a0 && nd.c0 >= 0, in1 = a1 && nd.c1 >= 0;
+        if (in0) {
+          ref = nd.c0;
+          if (in1) stack[sp++] = nd.c1;
+        } else if (in1) {
+          ref = nd.c1;
+        } else {
+          if (sp == 0) break;
+          ref = stack[--sp];
         }
       }
-      if (sp == 0) break;
-      ref = stack[--sp];
     }
   }
-  if constexpr (!FILL) counts[qi] = cnt;
+  if constexpr (FILL) { if (__any_sync(~0u, pend > 0)) flush(); }
+  else { if (valid) counts[qi] = cnt; }
 }
 
 // ---- K1 / K2: k nearest neighbours ------------------------------------------------------------------
@@ -281,6 +320,12 @@ struct LocalHeap {
   }
 };
 
+// Packet kNN: the warp walks the tree once for its 32 query points.  Every lane keeps its own
+// best-k set and prunes with its own k-th distance; the warp visits a child if ANY lane still
+// needs it and takes the child that more lanes find nearer first.  Leaf-range children are
+// scanned on the spot (their size is known from the node), internal children go on the
+// shared-memory stack; a popped node is re-tested against the current bounds through its
+// children's boxes.
 template <int PK, class Heap>
 __global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ nodes,
                                                  const float4* __restrict__ leaves,
@@ -289,51 +334,59 @@ __global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ node
                                                  const uint32_t* __restrict__ qorder, int64_t nq, int k,
                                                  int64_t n, int32_t* __restrict__ indices,
                                                  float* __restrict__ distances) {
+  __shared__ int32_t s_stack[QT / 32][STACK_DEPTH];
+  int32_t* stack = s_stack[threadIdx.x >> 5];
   const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
-  if (t >= nq) return;
-  const int64_t qi = qorder ? (int64_t)qorder[t] : t;
+  const bool valid = t < nq;
+  const int64_t qi = valid ? (qorder ? (int64_t)qorder[t] : t) : 0;
   float y[D];
 #pragma unroll
   for (int a = 0; a < D; ++a) y[a] = __ldg(qpoints + qi * D + a);
   Heap heap;
   heap.init(k);
+
+  auto leaf_range = [&](int first, int m) {   // m is warp-uniform
+#pragma unroll 2
+    for (int j = 0; j < m; ++j) {
+      Leaf<PK> lf;
+      load_leaf<PK>(leaves, first + j, lf);
+      const float key = knn_key<PK>(y, lf.v);
+      if (valid && key < heap.worst()) heap.push(key, (int32_t)(lf.idx & ~LEAF_END));
+    }
+  };
+
   if (n > 0) {
-    int32_t sref[STACK_DEPTH];
-    float sbound[STACK_DEPTH];
-    int sp = 0;
     int32_t ref = __ldg(root);
-    for (;;) {
-      if (ref >= 0) {
-        Node nd;
-        load_node(nodes, ref, nd);
-        float b0 = knn_bound<PK>(y, nd.v, nd.v + D);
-        float b1 = knn_bound<PK>(y, nd.v + 2 * D, nd.v + 3 * D);
-        int32_t c0 = nd.c0, c1 = nd.c1;
-        if (b1 < b0) { float tb = b0; b0 = b1; b1 = tb; int32_t tc = c0; c0 = c1; c1 = tc; }
-        const float w = heap.worst();
-        if (b0 < w) {
-          ref = c0;
-          if (b1 < w) { sref[sp] = c1; sbound[sp] = b1; ++sp; }
-          continue;
+    if (ref < 0) {
+      leaf_range(0, (int)n);
+    } else {
+      int sp = 0;
+      for (;;) {
+        NodeX nd;
+        load_node_x(nodes, ref, nd);
+        const float b0 = knn_bound<PK>(y, nd.v, nd.v + D);
+        const float b1 = knn_bound<PK>(y, nd.v + 2 * D, nd.v + 3 * D);
+        // child 1 first if more lanes find it nearer
+        const bool swap = __popc(__ballot_sync(~0u, valid && b1 < b0)) > __popc(__ballot_sync(~0u, valid && b0 < b1));
+        const float bn = swap ? b1 : b0, bf = swap ? b0 : b1;
+        const int32_t cn = swap ? nd.c1 : nd.c0, cf = swap ? nd.c0 : nd.c1;
+        int32_t next = -1;
+        if (__any_sync(~0u, valid && bn < heap.worst())) {
+          if (cn < 0) { if (swap) leaf_range(ref + 1, nd.r - ref); else leaf_range(nd.l, ref - nd.l + 1); }
+          else next = cn;
         }
-      } else {
-        int j = ~ref;
-        for (;; ++j) {
-          Leaf<PK> lf;
-          load_leaf<PK>(leaves, j, lf);
-          const float key = knn_key<PK>(y, lf.v);
-          if (key < heap.worst()) heap.push(key, (int32_t)(lf.idx & ~LEAF_END));
-          if (lf.idx & LEAF_END) break;
+        if (__any_sync(~0u, valid && bf < heap.worst())) {
+          if (cf < 0) { if (swap) leaf_range(nd.l, ref - nd.l + 1); else leaf_range(ref + 1, nd.r - ref); }
+          else if (next >= 0) stack[sp++] = cf;
+          else next = cf;
         }
+        if (next >= 0) { ref = next; continue; }
+        if (sp == 0) break;
+        ref = stack[--sp];
       }
-      bool found = false;
-      while (sp > 0) {
-        --sp;
-        if (sbound[sp] < heap.worst()) { ref = sref[sp]; found = true; break; }
-      }
-      if (!found) break;
     }
   }
+  if (!valid) return;
   int32_t* oi = indices + qi * k;
   float* od = distances ? distances + qi * k : nullptr;
   heap.emit(k, [&](int s, float key, int32_t idx) {
@@ -351,9 +404,9 @@ arbx_status spatial_launch(const Index* ix, const float* queries, int64_t nq, co
   const float4* leaves = reinterpret_cast<const float4*>(ix->leaves);
   ProfScope ps(indices ? K_SPATIAL_FILL : K_SPATIAL_COUNT, s);
   if (indices)
-    spatial_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
+    spatial_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices);
   else
-    spatial_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
+    spatial_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
