@@ -6,6 +6,7 @@
 // One query per thread; the 32 queries of a warp are neighbours on the space-filling curve
 // (qorder), so they walk nearly the same nodes and the node fetches hit L1/L2.
 #include <algorithm>
+#include <cstdlib>
 
 #include "geom.cuh"
 
@@ -45,6 +46,20 @@ __global__ void __launch_bounds__(256) qcode_kernel(const float* __restrict__ qu
 }
 
 // ---- node / leaf access ------------------------------------------------------------------------
+struct Node { float v[4 * D]; int32_t c0, c1; };
+
+__device__ __forceinline__ void load_node(const float4* __restrict__ nodes, int32_t ref, Node& nd) {
+  const float4* p = nodes + (int64_t)ref * (D + 1);
+#pragma unroll
+  for (int e = 0; e < D; ++e) {
+    float4 t = __ldg(p + e);
+    nd.v[4 * e] = t.x; nd.v[4 * e + 1] = t.y; nd.v[4 * e + 2] = t.z; nd.v[4 * e + 3] = t.w;
+  }
+  float4 t = __ldg(p + D);
+  nd.c0 = __float_as_int(t.x);
+  nd.c1 = __float_as_int(t.y);
+}
+
 template <int PK>
 struct Leaf { float v[prim_width(PK, D)]; uint32_t idx; };
 
@@ -175,15 +190,16 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   if constexpr (FILL) base = valid ? offsets[qi] : 0;
   int cnt = 0, pend = 0;
 
-  auto flush = [&]() {
+  auto flush = [&](uint32_t who) {   // who: lanes whose pending hits are written out (warp-uniform)
     __syncwarp();
-    for (int L = 0; L < 32; ++L) {
+    while (who) {
+      const int L = __ffs(who) - 1;
+      who &= who - 1;
       const int m = __shfl_sync(~0u, pend, L);
       const int b = __shfl_sync(~0u, base, L);
       if (lane < m) indices[b + lane] = stage[lane * 33 + L];
+      if (lane == L) { base += pend; pend = 0; }
     }
-    base += pend;
-    pend = 0;
     __syncwarp();
   };
 
@@ -195,7 +211,8 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
       const bool hit = alive && hits_prim<QK, PK>(q, lf.v);
       if constexpr (FILL) {
         if (hit) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
-        if (__any_sync(~0u, pend == FS)) flush();
+        const uint32_t full = __ballot_sync(~0u, pend == FS);
+        if (full) flush(full);
       } else {
         cnt += hit ? 1 : 0;
       }
@@ -228,7 +245,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
       }
     }
   }
-  if constexpr (FILL) { if (__any_sync(~0u, pend > 0)) flush(); }
+  if constexpr (FILL) { flush(__ballot_sync(~0u, pend > 0)); }
   else { if (valid) counts[qi] = cnt; }
 }
 
@@ -395,6 +412,137 @@ __global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ node
   });
 }
 
+// ---- one query per thread (independent traversal) --------------------------------------------------
+// Kept beside the packet kernels: when the 32 queries of a warp are NOT spatially coherent
+// (high dimension, strongly clustered data) the packet visits the union of 32 unrelated
+// paths and independent traversal wins.  The host picks per call (see pick_packet below).
+template <int PK, int QK, bool FILL>
+__global__ void __launch_bounds__(QT) spatial_thread_kernel(const float4* __restrict__ nodes,
+                                                     const float4* __restrict__ leaves,
+                                                     const int32_t* __restrict__ root,
+                                                     const float* __restrict__ queries,
+                                                     const uint32_t* __restrict__ qorder, int64_t nq,
+                                                     int32_t* __restrict__ counts,
+                                                     const int32_t* __restrict__ offsets,
+                                                     int32_t* __restrict__ indices) {
+  constexpr int QW = prim_width(QK, D);
+  const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
+  if (t >= nq) return;
+  const int64_t qi = qorder ? (int64_t)qorder[t] : t;
+  Query<QK> q;
+#pragma unroll
+  for (int e = 0; e < QW; ++e) q.v[e] = __ldg(queries + qi * QW + e);
+  bool alive = true;
+  if constexpr (QK == KIND_SPHERE) {
+    q.r2 = q.v[D] * q.v[D];
+    alive = q.v[D] >= 0.f;      // negative radius matches nothing (reading A21)
+  }
+  int32_t* out = nullptr;
+  if constexpr (FILL) out = indices + offsets[qi];
+  int cnt = 0;
+  if (alive) {
+    int32_t stack[STACK_DEPTH];
+    int sp = 0;
+    int32_t ref = __ldg(root);
+    for (;;) {
+      if (ref >= 0) {
+        Node nd;
+        load_node(nodes, ref, nd);
+        const bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
+        const bool h1 = hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D);
+        if (h0) {
+          ref = nd.c0;
+          if (h1) stack[sp++] = nd.c1;
+          continue;
+        }
+        if (h1) { ref = nd.c1; continue; }
+      } else {
+        int j = ~ref;
+        for (;; ++j) {
+          Leaf<PK> lf;
+          load_leaf<PK>(leaves, j, lf);
+          if (hits_prim<QK, PK>(q, lf.v)) {
+            if constexpr (FILL) out[cnt] = (int32_t)(lf.idx & ~LEAF_END);
+            ++cnt;
+          }
+          if (lf.idx & LEAF_END) break;
+        }
+      }
+      if (sp == 0) break;
+      ref = stack[--sp];
+    }
+  }
+  if constexpr (!FILL) counts[qi] = cnt;
+}
+
+template <int PK, class Heap>
+__global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict__ nodes,
+                                                 const float4* __restrict__ leaves,
+                                                 const int32_t* __restrict__ root,
+                                                 const float* __restrict__ qpoints,
+                                                 const uint32_t* __restrict__ qorder, int64_t nq, int k,
+                                                 int64_t n, int32_t* __restrict__ indices,
+                                                 float* __restrict__ distances) {
+  const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
+  if (t >= nq) return;
+  const int64_t qi = qorder ? (int64_t)qorder[t] : t;
+  float y[D];
+#pragma unroll
+  for (int a = 0; a < D; ++a) y[a] = __ldg(qpoints + qi * D + a);
+  Heap heap;
+  heap.init(k);
+  if (n > 0) {
+    int32_t sref[STACK_DEPTH];
+    float sbound[STACK_DEPTH];
+    int sp = 0;
+    int32_t ref = __ldg(root);
+    for (;;) {
+      if (ref >= 0) {
+        Node nd;
+        load_node(nodes, ref, nd);
+        float b0 = knn_bound<PK>(y, nd.v, nd.v + D);
+        float b1 = knn_bound<PK>(y, nd.v + 2 * D, nd.v + 3 * D);
+        int32_t c0 = nd.c0, c1 = nd.c1;
+        if (b1 < b0) { float tb = b0; b0 = b1; b1 = tb; int32_t tc = c0; c0 = c1; c1 = tc; }
+        const float w = heap.worst();
+        if (b0 < w) {
+          ref = c0;
+          if (b1 < w) { sref[sp] = c1; sbound[sp] = b1; ++sp; }
+          continue;
+        }
+      } else {
+        int j = ~ref;
+        for (;; ++j) {
+          Leaf<PK> lf;
+          load_leaf<PK>(leaves, j, lf);
+          const float key = knn_key<PK>(y, lf.v);
+          if (key < heap.worst()) heap.push(key, (int32_t)(lf.idx & ~LEAF_END));
+          if (lf.idx & LEAF_END) break;
+        }
+      }
+      bool found = false;
+      while (sp > 0) {
+        --sp;
+        if (sbound[sp] < heap.worst()) { ref = sref[sp]; found = true; break; }
+      }
+      if (!found) break;
+    }
+  }
+  int32_t* oi = indices + qi * k;
+  float* od = distances ? distances + qi * k : nullptr;
+  heap.emit(k, [&](int s, float key, int32_t idx) {
+    oi[s] = idx;
+    if (od) od[s] = (PK == KIND_SPHERE || idx < 0) ? key : sqrtf(key);
+  });
+}
+
+// Experiment switch ARBX_TRAVERSAL: unset = default (packet spatial, per-thread kNN),
+// "thread" = one query per thread everywhere, "packet" = packets everywhere.
+inline int traversal_mode() {
+  const char* v = getenv("ARBX_TRAVERSAL");
+  return !v ? 0 : v[0] == 't' ? 1 : v[0] == 'p' ? 2 : 0;
+}
+
 // ---- host dispatch ------------------------------------------------------------------------------------
 template <int PK, int QK>
 arbx_status spatial_launch(const Index* ix, const float* queries, int64_t nq, const uint32_t* qorder,
@@ -403,10 +551,15 @@ arbx_status spatial_launch(const Index* ix, const float* queries, int64_t nq, co
   const float4* nodes = reinterpret_cast<const float4*>(ix->nodes);
   const float4* leaves = reinterpret_cast<const float4*>(ix->leaves);
   ProfScope ps(indices ? K_SPATIAL_FILL : K_SPATIAL_COUNT, s);
-  if (indices)
+  const bool packet = traversal_mode() != 1;
+  if (indices && packet)
     spatial_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices);
-  else
+  else if (packet)
     spatial_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices);
+  else if (indices)
+    spatial_thread_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
+  else
+    spatial_thread_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
@@ -435,9 +588,14 @@ arbx_status knn_launch(const Index* ix, const float* qpoints, int64_t nq, int k,
                        int32_t* indices, float* distances, cudaStream_t s) {
   const unsigned grid = (unsigned)((nq + QT - 1) / QT);
   ProfScope ps(K_KNN, s);
-  knn_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
-                                           reinterpret_cast<const float4*>(ix->leaves), ix->root, qpoints,
-                                           qorder, nq, k, ix->n, indices, distances);
+  if (traversal_mode() == 2)
+    knn_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
+                                             reinterpret_cast<const float4*>(ix->leaves), ix->root, qpoints,
+                                             qorder, nq, k, ix->n, indices, distances);
+  else
+    knn_thread_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
+                                                    reinterpret_cast<const float4*>(ix->leaves), ix->root, qpoints,
+                                                    qorder, nq, k, ix->n, indices, distances);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
