@@ -24,7 +24,7 @@ constexpr int QT = 128;   // threads per block of the traversal kernels
 template <int QK>
 __global__ void __launch_bounds__(256) qcode_kernel(const float* __restrict__ queries, int64_t nq,
                                                     const float* __restrict__ bounds,
-                                                    uint32_t* __restrict__ codes) {
+                                                    uint32_t* __restrict__ codes, int drop) {
   constexpr int QW = prim_width(QK, D);
   constexpr int B = qcode_bits_per_axis(D);
   float lo[D], scale[D];
@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) qcode_kernel(const float* __restrict__ qu
     centre_of<D, QK>(v, c);
     uint32_t q[D];
     quantise<D, B>(c, lo, scale, q);
-    codes[i] = interleave<D, B, uint32_t>(q);
+    codes[i] = interleave<D, B, uint32_t>(q) >> drop;
   }
 }
 
@@ -203,18 +203,26 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
     __syncwarp();
   };
 
+  constexpr int CH = 4;     // FILL: staging room is checked once per CH primitives
   auto leaf_range = [&](int first, int m) {   // m is warp-uniform
-#pragma unroll 4
-    for (int j = 0; j < m; ++j) {
-      Leaf<PK> lf;
-      load_leaf<PK>(leaves, first + j, lf);
-      const bool hit = alive && hits_prim<QK, PK>(q, lf.v);
-      if constexpr (FILL) {
-        if (hit) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
-        const uint32_t full = __ballot_sync(~0u, pend == FS);
+    if constexpr (FILL) {
+      for (int j0 = 0; j0 < m; j0 += CH) {
+        const uint32_t full = __ballot_sync(~0u, pend > FS - CH);
         if (full) flush(full);
-      } else {
-        cnt += hit ? 1 : 0;
+        const int je = min(m, j0 + CH);
+#pragma unroll 4
+        for (int j = j0; j < je; ++j) {
+          Leaf<PK> lf;
+          load_leaf<PK>(leaves, first + j, lf);
+          if (alive && hits_prim<QK, PK>(q, lf.v)) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
+        }
+      }
+    } else {
+#pragma unroll 4
+      for (int j = 0; j < m; ++j) {
+        Leaf<PK> lf;
+        load_leaf<PK>(leaves, first + j, lf);
+        cnt += (alive && hits_prim<QK, PK>(q, lf.v)) ? 1 : 0;
       }
     }
   };
@@ -292,6 +300,20 @@ struct RegHeap {
     for (int s = 0; s < KB; ++s)
       if (s >= KB - k) f(s - (KB - k), d[s], i[s]);
   }
+  // k == KB and KB % 4 == 0: the row is 16-byte aligned, write it with 128-bit stores
+  static constexpr bool kVec = KB % 4 == 0;
+  static constexpr int kSlots = KB;
+  __device__ __forceinline__ void emit_vec(int32_t* oi, float* od, bool take_sqrt) {
+#pragma unroll
+    for (int s = 0; s < KB / 4; ++s) {
+      reinterpret_cast<int4*>(oi)[s] = make_int4(i[4 * s], i[4 * s + 1], i[4 * s + 2], i[4 * s + 3]);
+      if (od) {
+        float4 v = make_float4(d[4 * s], d[4 * s + 1], d[4 * s + 2], d[4 * s + 3]);
+        if (take_sqrt) { v.x = sqrtf(v.x); v.y = sqrtf(v.y); v.z = sqrtf(v.z); v.w = sqrtf(v.w); }
+        reinterpret_cast<float4*>(od)[s] = v;
+      }
+    }
+  }
 };
 
 // k > 32: binary max-heap in local memory, heap-sorted at the end
@@ -326,6 +348,9 @@ struct LocalHeap {
       sift_down(0, k, t, idx);
     }
   }
+  static constexpr bool kVec = false;
+  static constexpr int kSlots = 0;
+  __device__ __forceinline__ void emit_vec(int32_t*, float*, bool) {}
   template <class F>
   __device__ __forceinline__ void emit(int kk, F&& f) {
     for (int size = m; size > 1; --size) {   // heap sort: largest to the back
@@ -363,12 +388,20 @@ __global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ node
   heap.init(k);
 
   auto leaf_range = [&](int first, int m) {   // m is warp-uniform
-#pragma unroll 2
-    for (int j = 0; j < m; ++j) {
-      Leaf<PK> lf;
-      load_leaf<PK>(leaves, first + j, lf);
-      const float key = knn_key<PK>(y, lf.v);
-      if (valid && key < heap.worst()) heap.push(key, (int32_t)(lf.idx & ~LEAF_END));
+    constexpr int CH = 4;   // the loads and keys of a chunk are independent of its pushes
+    for (int j0 = 0; j0 < m; j0 += CH) {
+      float key[CH];
+      int32_t id[CH];
+#pragma unroll
+      for (int j = 0; j < CH; ++j) {
+        Leaf<PK> lf;
+        load_leaf<PK>(leaves, min(first + j0 + j, first + m - 1), lf);
+        key[j] = j0 + j < m ? knn_key<PK>(y, lf.v) : INFINITY;
+        id[j] = (int32_t)(lf.idx & ~LEAF_END);
+      }
+#pragma unroll
+      for (int j = 0; j < CH; ++j)
+        if (valid && key[j] < heap.worst()) heap.push(key[j], id[j]);
     }
   };
 
@@ -406,6 +439,10 @@ __global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ node
   if (!valid) return;
   int32_t* oi = indices + qi * k;
   float* od = distances ? distances + qi * k : nullptr;
+  if constexpr (Heap::kVec) {
+    // sqrt(+inf) = +inf keeps the padding of short rows (n < k) intact
+    if (k == Heap::kSlots) { heap.emit_vec(oi, od, PK != KIND_SPHERE); return; }
+  }
   heap.emit(k, [&](int s, float key, int32_t idx) {
     oi[s] = idx;
     if (od) od[s] = (PK == KIND_SPHERE || idx < 0) ? key : sqrtf(key);
@@ -530,6 +567,10 @@ __global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict
   }
   int32_t* oi = indices + qi * k;
   float* od = distances ? distances + qi * k : nullptr;
+  if constexpr (Heap::kVec) {
+    // sqrt(+inf) = +inf keeps the padding of short rows (n < k) intact
+    if (k == Heap::kSlots) { heap.emit_vec(oi, od, PK != KIND_SPHERE); return; }
+  }
   heap.emit(k, [&](int s, float key, int32_t idx) {
     oi[s] = idx;
     if (od) od[s] = (PK == KIND_SPHERE || idx < 0) ? key : sqrtf(key);
@@ -628,13 +669,18 @@ arbx_status qcode_entry(const Index* ix, const float* queries, int64_t nq, int q
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((nq + 255) / 256, (int64_t)sms * 8));
   ProfScope ps(K_QCODE, s);
+  // the sort key keeps the top `qb` bits per axis of the code (whole 8-bit digit passes)
+  constexpr int B = qcode_bits_per_axis(D);
+  int qb = B;
+  if (const char* v = getenv("ARBX_QBITS")) qb = std::max(1, std::min(B, atoi(v)));
+  const int drop = D * (B - qb);
   switch (qkind) {
-    case KIND_POINT: qcode_kernel<KIND_POINT><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes); break;
-    case KIND_BOX: qcode_kernel<KIND_BOX><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes); break;
-    default: qcode_kernel<KIND_SPHERE><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes); break;
+    case KIND_POINT: qcode_kernel<KIND_POINT><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes, drop); break;
+    case KIND_BOX: qcode_kernel<KIND_BOX><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes, drop); break;
+    default: qcode_kernel<KIND_SPHERE><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes, drop); break;
   }
   ARBX_LAUNCH_CHECK();
-  *key_bits = D * qcode_bits_per_axis(D);
+  *key_bits = D * qb;
   return ARBX_OK;
 }
 

@@ -116,22 +116,28 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
     if constexpr (VALS) val[j] = IOTA ? idx : (idx < n ? vin[idx] : 0u);
   }
 
-  // stable rank of every key among the keys of its warp with the same digit
+  // stable rank of every key among the keys of its warp with the same digit.  The match
+  // instructions of a batch are independent (their latency overlaps); the per-digit counters
+  // are bumped by one leader lane per digit group with a shared-memory atomic, and program
+  // order inside the warp keeps item j ahead of item j+1.
   uint16_t rank[SORT_IPT];
   const uint32_t lt_mask = (1u << lane) - 1u;
+  constexpr int MB = 8;
 #pragma unroll
-  for (int j = 0; j < SORT_IPT; ++j) {
-    const uint32_t d = (uint32_t)(key[j] >> shift) & 255u;
-    const uint32_t peers = __match_any_sync(~0u, d);
-    const int leader = __ffs(peers) - 1;
-    uint32_t old = 0;
-    if (lane == leader) {
-      old = whist[w][d];
-      whist[w][d] = old + __popc(peers);
+  for (int j0 = 0; j0 < SORT_IPT; j0 += MB) {
+    uint32_t peers[MB];
+#pragma unroll
+    for (int j = 0; j < MB; ++j)
+      peers[j] = __match_any_sync(~0u, (uint32_t)(key[j0 + j] >> shift) & 255u);
+#pragma unroll
+    for (int j = 0; j < MB; ++j) {
+      const uint32_t d = (uint32_t)(key[j0 + j] >> shift) & 255u;
+      const int leader = __ffs(peers[j]) - 1;
+      uint32_t old = 0;
+      if (lane == leader) old = atomicAdd(&whist[w][d], (uint32_t)__popc(peers[j]));
+      old = __shfl_sync(~0u, old, leader);
+      rank[j0 + j] = (uint16_t)(old + __popc(peers[j] & lt_mask));
     }
-    old = __shfl_sync(~0u, old, leader);
-    rank[j] = (uint16_t)(old + __popc(peers & lt_mask));
-    __syncwarp();
   }
   __syncthreads();
 
