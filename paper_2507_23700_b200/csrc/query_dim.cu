@@ -7,6 +7,7 @@
 // (qorder), so they walk nearly the same nodes and the node fetches hit L1/L2.
 #include <algorithm>
 #include <cstdlib>
+#include <cstdint>
 
 #include "geom.cuh"
 
@@ -532,9 +533,20 @@ __global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict
     int32_t sref[STACK_DEPTH];
     float sbound[STACK_DEPTH];
     int sp = 0;
+    constexpr int32_t DONE = INT32_MIN;
+    auto pop = [&]() -> int32_t {
+      while (sp > 0) {
+        --sp;
+        if (sbound[sp] < heap.worst()) return sref[sp];
+      }
+      return DONE;
+    };
     int32_t ref = __ldg(root);
+    // "while-while" loop: all lanes first descend through internal nodes until each holds a
+    // leaf range (or is done), then the leaf scans run together -- less divergence than
+    // mixing node steps and leaf scans in one loop body.
     for (;;) {
-      if (ref >= 0) {
+      while (ref >= 0) {
         Node nd;
         load_node(nodes, ref, nd);
         float b0 = knn_bound<PK>(y, nd.v, nd.v + D);
@@ -545,24 +557,20 @@ __global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict
         if (b0 < w) {
           ref = c0;
           if (b1 < w) { sref[sp] = c1; sbound[sp] = b1; ++sp; }
-          continue;
-        }
-      } else {
-        int j = ~ref;
-        for (;; ++j) {
-          Leaf<PK> lf;
-          load_leaf<PK>(leaves, j, lf);
-          const float key = knn_key<PK>(y, lf.v);
-          if (key < heap.worst()) heap.push(key, (int32_t)(lf.idx & ~LEAF_END));
-          if (lf.idx & LEAF_END) break;
+        } else {
+          ref = pop();
         }
       }
-      bool found = false;
-      while (sp > 0) {
-        --sp;
-        if (sbound[sp] < heap.worst()) { ref = sref[sp]; found = true; break; }
+      if (ref == DONE) break;
+      int j = ~ref;
+      for (;; ++j) {
+        Leaf<PK> lf;
+        load_leaf<PK>(leaves, j, lf);
+        const float key = knn_key<PK>(y, lf.v);
+        if (key < heap.worst()) heap.push(key, (int32_t)(lf.idx & ~LEAF_END));
+        if (lf.idx & LEAF_END) break;
       }
-      if (!found) break;
+      ref = pop();
     }
   }
   int32_t* oi = indices + qi * k;
