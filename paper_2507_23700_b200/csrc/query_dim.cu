@@ -143,6 +143,72 @@ __device__ __forceinline__ bool hits_prim(const Query<QK>& q, const float* p) {
 // instead of 32 divergent ones, control flow is uniform, and the stack is one short array
 // per warp in shared memory.  The leaf test is per lane and exact, so the result is the same
 // set as one-query-per-thread traversal.
+template <int PK, int QK, bool FILL>
+__device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes, const float4* __restrict__ leaves,
+                                               const int32_t* __restrict__ root, const Query<QK>& q,
+                                               int32_t* __restrict__ out) {
+  int cnt = 0;
+  int32_t stack[STACK_DEPTH];
+  int sp = 0;
+  constexpr int32_t DONE = INT32_MIN;
+  int32_t ref = __ldg(root);
+  for (;;) {   // while-while: descend to a leaf range in every lane, then scan together
+    while (ref >= 0) {
+      Node nd;
+      load_node(nodes, ref, nd);
+      const bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
+      const bool h1 = hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D);
+      if (h0) {
+        ref = nd.c0;
+        if (h1) stack[sp++] = nd.c1;
+      } else if (h1) {
+        ref = nd.c1;
+      } else {
+        ref = sp > 0 ? stack[--sp] : DONE;
+      }
+    }
+    if (ref == DONE) break;
+    int j = ~ref;
+    for (;; ++j) {
+      Leaf<PK> lf;
+      load_leaf<PK>(leaves, j, lf);
+      if (hits_prim<QK, PK>(q, lf.v)) {
+        if constexpr (FILL) out[cnt] = (int32_t)(lf.idx & ~LEAF_END);
+        ++cnt;
+      }
+      if (lf.idx & LEAF_END) break;
+    }
+    ref = sp > 0 ? stack[--sp] : DONE;
+  }
+  return cnt;
+}
+
+// Are the 32 queries of this warp close together compared with their own reach?  Per axis:
+// spread of the query centres <= alpha * (largest query extent).  Coherent warps take the
+// packet path, the others traverse independently (one query per lane).  Warp-uniform result.
+template <int QK>
+__device__ __forceinline__ bool warp_coherent(const Query<QK>& q, bool valid, float alpha) {
+  if constexpr (QK == KIND_POINT) {
+    return false;
+  } else {
+    bool ok = true;
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+      const float c = QK == KIND_BOX ? 0.5f * q.v[a] + 0.5f * q.v[D + a] : q.v[a];
+      const float ext = QK == KIND_BOX ? q.v[D + a] - q.v[a] : 2.f * q.v[D];
+      float lo = valid ? c : INFINITY, hi = valid ? c : -INFINITY, e = valid ? ext : 0.f;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        lo = fminf(lo, __shfl_xor_sync(~0u, lo, o));
+        hi = fmaxf(hi, __shfl_xor_sync(~0u, hi, o));
+        e = fmaxf(e, __shfl_xor_sync(~0u, e, o));
+      }
+      ok = ok && (hi - lo <= alpha * e);
+    }
+    return ok;
+  }
+}
+
 struct NodeX { float v[4 * D]; int32_t c0, c1, l, r; };
 
 __device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, int32_t ref, NodeX& nd) {
@@ -165,7 +231,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
                                                      const uint32_t* __restrict__ qorder, int64_t nq,
                                                      int32_t* __restrict__ counts,
                                                      const int32_t* __restrict__ offsets,
-                                                     int32_t* __restrict__ indices) {
+                                                     int32_t* __restrict__ indices, int mode, float alpha) {
   constexpr int QW = prim_width(QK, D);
   __shared__ int32_t s_stack[QT / 32][STACK_DEPTH];
   int32_t* stack = s_stack[threadIdx.x >> 5];
@@ -179,6 +245,13 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   if constexpr (QK == KIND_SPHERE) {
     q.r2 = q.v[D] * q.v[D];
     alive = alive && q.v[D] >= 0.f;      // negative radius matches nothing (reading A21)
+  }
+  // mode 0: per-warp choice; 1: always one query per lane; 2: always packet
+  if (mode == 1 || (mode == 0 && !warp_coherent<QK>(q, valid, alpha))) {
+    int c = 0;
+    if (alive) c = thread_traverse<PK, QK, FILL>(nodes, leaves, root, q, FILL ? indices + offsets[qi] : nullptr);
+    if constexpr (!FILL) { if (valid) counts[qi] = c; }
+    return;
   }
   // FILL: hits are staged per lane in shared memory (FS slots, column `lane` of a padded
   // [FS][33] array) and flushed row by row with all lanes writing one query's pending hits as
@@ -454,65 +527,6 @@ __global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ node
 // Kept beside the packet kernels: when the 32 queries of a warp are NOT spatially coherent
 // (high dimension, strongly clustered data) the packet visits the union of 32 unrelated
 // paths and independent traversal wins.  The host picks per call (see pick_packet below).
-template <int PK, int QK, bool FILL>
-__global__ void __launch_bounds__(QT) spatial_thread_kernel(const float4* __restrict__ nodes,
-                                                     const float4* __restrict__ leaves,
-                                                     const int32_t* __restrict__ root,
-                                                     const float* __restrict__ queries,
-                                                     const uint32_t* __restrict__ qorder, int64_t nq,
-                                                     int32_t* __restrict__ counts,
-                                                     const int32_t* __restrict__ offsets,
-                                                     int32_t* __restrict__ indices) {
-  constexpr int QW = prim_width(QK, D);
-  const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
-  if (t >= nq) return;
-  const int64_t qi = qorder ? (int64_t)qorder[t] : t;
-  Query<QK> q;
-#pragma unroll
-  for (int e = 0; e < QW; ++e) q.v[e] = __ldg(queries + qi * QW + e);
-  bool alive = true;
-  if constexpr (QK == KIND_SPHERE) {
-    q.r2 = q.v[D] * q.v[D];
-    alive = q.v[D] >= 0.f;      // negative radius matches nothing (reading A21)
-  }
-  int32_t* out = nullptr;
-  if constexpr (FILL) out = indices + offsets[qi];
-  int cnt = 0;
-  if (alive) {
-    int32_t stack[STACK_DEPTH];
-    int sp = 0;
-    int32_t ref = __ldg(root);
-    for (;;) {
-      if (ref >= 0) {
-        Node nd;
-        load_node(nodes, ref, nd);
-        const bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
-        const bool h1 = hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D);
-        if (h0) {
-          ref = nd.c0;
-          if (h1) stack[sp++] = nd.c1;
-          continue;
-        }
-        if (h1) { ref = nd.c1; continue; }
-      } else {
-        int j = ~ref;
-        for (;; ++j) {
-          Leaf<PK> lf;
-          load_leaf<PK>(leaves, j, lf);
-          if (hits_prim<QK, PK>(q, lf.v)) {
-            if constexpr (FILL) out[cnt] = (int32_t)(lf.idx & ~LEAF_END);
-            ++cnt;
-          }
-          if (lf.idx & LEAF_END) break;
-        }
-      }
-      if (sp == 0) break;
-      ref = stack[--sp];
-    }
-  }
-  if constexpr (!FILL) counts[qi] = cnt;
-}
-
 template <int PK, class Heap>
 __global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict__ nodes,
                                                  const float4* __restrict__ leaves,
@@ -600,15 +614,13 @@ arbx_status spatial_launch(const Index* ix, const float* queries, int64_t nq, co
   const float4* nodes = reinterpret_cast<const float4*>(ix->nodes);
   const float4* leaves = reinterpret_cast<const float4*>(ix->leaves);
   ProfScope ps(indices ? K_SPATIAL_FILL : K_SPATIAL_COUNT, s);
-  const bool packet = traversal_mode() != 1;
-  if (indices && packet)
-    spatial_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices);
-  else if (packet)
-    spatial_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices);
-  else if (indices)
-    spatial_thread_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
+  const int mode = traversal_mode();
+  float alpha = 0.75f;
+  if (const char* v = getenv("ARBX_PACKET_ALPHA")) alpha = (float)atof(v);
+  if (indices)
+    spatial_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices, mode, alpha);
   else
-    spatial_thread_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, queries, qorder, nq, counts, offsets, indices);
+    spatial_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices, mode, alpha);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
