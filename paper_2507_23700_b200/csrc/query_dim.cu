@@ -359,6 +359,31 @@ struct RegHeap {
   }
   __device__ __forceinline__ float worst() const { return d[KB - 1]; }
   __device__ __forceinline__ void push(float t, int32_t idx) {   // requires t < worst()
+    if constexpr (KB >= 16) {
+      constexpr int H = KB / 2;
+      if (t >= d[H - 1]) {      // lands in the upper half: the lower half is untouched
+        d[KB - 1] = t; i[KB - 1] = idx;
+#pragma unroll
+        for (int s = KB - 1; s > H; --s) {
+          const bool sw = d[s] < d[s - 1];
+          const float td = d[s]; const int32_t ti = i[s];
+          d[s] = sw ? d[s - 1] : td; i[s] = sw ? i[s - 1] : ti;
+          d[s - 1] = sw ? td : d[s - 1]; i[s - 1] = sw ? ti : i[s - 1];
+        }
+        return;
+      }
+#pragma unroll
+      for (int s = KB - 1; s >= H; --s) { d[s] = d[s - 1]; i[s] = i[s - 1]; }   // upper half moves up by one
+      d[H - 1] = t; i[H - 1] = idx;
+#pragma unroll
+      for (int s = H - 1; s > 0; --s) {
+        const bool sw = d[s] < d[s - 1];
+        const float td = d[s]; const int32_t ti = i[s];
+        d[s] = sw ? d[s - 1] : td; i[s] = sw ? i[s - 1] : ti;
+        d[s - 1] = sw ? td : d[s - 1]; i[s - 1] = sw ? ti : i[s - 1];
+      }
+      return;
+    }
     d[KB - 1] = t; i[KB - 1] = idx;
 #pragma unroll
     for (int s = KB - 1; s > 0; --s) {
