@@ -30,6 +30,19 @@ __device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v) {
   asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
+// lanes of the warp holding the same 8-bit digit: eight ballots, one per bit (plain ALU/vote
+// work; the match.any instruction is far slower than this on sm_100)
+__device__ __forceinline__ uint32_t match_digit(uint32_t d) {
+  uint32_t peers = ~0u;
+#pragma unroll
+  for (int b = 0; b < 8; ++b) {
+    const bool bit = (d >> b) & 1u;
+    const uint32_t bal = __ballot_sync(~0u, bit);
+    peers &= bit ? bal : ~bal;
+  }
+  return peers;
+}
+
 // ---- histogram of every digit in one read of the keys ---------------------------------------
 template <typename K>
 __global__ void __launch_bounds__(512) hist_kernel(const K* __restrict__ keys, uint32_t n, int npass,
@@ -128,7 +141,7 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
     uint32_t peers[MB];
 #pragma unroll
     for (int j = 0; j < MB; ++j)
-      peers[j] = __match_any_sync(~0u, (uint32_t)(key[j0 + j] >> shift) & 255u);
+      peers[j] = match_digit((uint32_t)(key[j0 + j] >> shift) & 255u);
 #pragma unroll
     for (int j = 0; j < MB; ++j) {
       const uint32_t d = (uint32_t)(key[j0 + j] >> shift) & 255u;
