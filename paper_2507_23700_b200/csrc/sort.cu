@@ -186,13 +186,29 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
 
     uint32_t excl = 0;
     if (tile > 0) {
+      // decoupled look-back, LB predecessors per round trip: the loads of a batch are
+      // independent, so a walk over many aggregate-only tiles costs one latency per batch
+      constexpr int LB = 8;
       int t = (int)tile - 1;
-      for (;;) {
-        uint32_t v;
-        do { v = ld_volatile_u32(&status[(size_t)t * RADIX + d]); } while ((v >> 30) == 0u);
-        excl += v & VAL_MASK;
-        if ((v >> 30) == 2u) break;
-        --t;
+      bool done = false;
+      while (!done) {
+        uint32_t v[LB];
+#pragma unroll
+        for (int i = 0; i < LB; ++i)
+          v[i] = t - i >= 0 ? ld_volatile_u32(&status[(size_t)(t - i) * RADIX + d]) : FLAG_INCL;
+        int used = 0;
+#pragma unroll
+        for (int i = 0; i < LB; ++i) {
+          if (!done && used == i) {
+            const uint32_t f = v[i] >> 30;
+            if (f != 0u) {            // published: take it; an inclusive prefix ends the walk
+              excl += v[i] & VAL_MASK;
+              used = i + 1;
+              done = f == 2u;
+            }
+          }
+        }
+        t -= used;                    // resume at the first predecessor that was not ready
       }
       st_volatile_u32(&status[(size_t)tile * RADIX + d], FLAG_INCL | (excl + pub));
     }
