@@ -200,7 +200,8 @@ arbx_status arbx_query_count(arbx_handle h, const float* queries, int64_t nq, ar
   if (ix->n == 0) { ARBX_CUDA(cudaMemsetAsync(counts, 0, (size_t)nq * sizeof(int32_t), s)); return ARBX_OK; }
   Scratch<uint32_t> order;
   ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
-  return dim_table(ix->dim)->spatial(ix, queries, nq, (int)qkind, order.p, counts, nullptr, nullptr, s);
+  SpatialArgs a{queries, nq, (int)qkind, order.p, counts, nullptr, nullptr, nullptr, 0, nullptr, 0};
+  return dim_table(ix->dim)->spatial(ix, a, s);
 }
 
 arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
@@ -219,17 +220,35 @@ arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, 
     return ARBX_OK;
   }
   Scratch<uint32_t> order;
-  Scratch<int32_t> counts;
-  Scratch<long long> total_dev;
+  Scratch<int32_t> counts, rows;
+  Scratch<long long> total_dev;   // [0] total, [1] number of queries with more than `cap` matches
   ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
   ARBX_TRY(counts.alloc((size_t)nq, s));
-  ARBX_TRY(total_dev.alloc(1, s));
+  ARBX_TRY(total_dev.alloc(2, s));
+  ARBX_CUDA(cudaMemsetAsync(total_dev.p, 0, 2 * sizeof(long long), s));
   const DimTable* tab = dim_table(ix->dim);
-  ARBX_TRY(tab->spatial(ix, queries, nq, (int)qkind, order.p, counts.p, nullptr, nullptr, s));
+  // Single traversal when the caller wants the indices: the count pass also stores the first
+  // `cap` matches of every query in a scratch row; after the scan the rows are copied into
+  // their CSR slices and only queries with more than cap matches are traversed again.
+  int cap = 0;
+  if (indices) {
+    const long long budget = (long long)env_int("ARBX_STORE_BUDGET_MB", 4096) << 20;
+    for (int c = 64; c >= 16 && cap == 0; c >>= 1)
+      if ((long long)nq * c * 4 <= budget) cap = c;
+  }
+  SpatialArgs a{queries, nq, (int)qkind, order.p, counts.p, nullptr, nullptr, nullptr, cap,
+                reinterpret_cast<int*>(total_dev.p + 1), cap ? 2 : 0};
+  if (cap) {
+    ARBX_TRY(rows.alloc((size_t)nq * cap, s));
+    a.rows = rows.p;
+  }
+  ARBX_TRY(tab->spatial(ix, a, s));
   ARBX_TRY(exclusive_scan_i32(counts.p, offsets, nq, total_dev.p, s));
-  long long total = 0;
-  ARBX_CUDA(cudaMemcpyAsync(&total, total_dev.p, sizeof(total), cudaMemcpyDeviceToHost, s));
+  long long host[2] = {0, 0};
+  ARBX_CUDA(cudaMemcpyAsync(host, total_dev.p, sizeof(host), cudaMemcpyDeviceToHost, s));
   ARBX_CUDA(cudaStreamSynchronize(s));
+  const long long total = host[0];
+  const int noverflow = (int)(host[1] & 0xffffffffLL);
   if (total_host) *total_host = total;
   if (total > 0x7fffffffLL) {
     set_error("arbx_query_spatial: total %lld exceeds INT32_MAX", total);
@@ -241,7 +260,14 @@ arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, 
     return ARBX_ERR_CAPACITY;
   }
   if (total == 0) return ARBX_OK;
-  return tab->spatial(ix, queries, nq, (int)qkind, order.p, nullptr, offsets, indices, s);
+  a.offsets = offsets;
+  a.indices = indices;
+  a.pass = 1;
+  if (cap) {
+    ARBX_TRY(compact_rows(rows.p, cap, counts.p, offsets, indices, nq, s));
+    if (noverflow == 0) return ARBX_OK;
+  }
+  return tab->spatial(ix, a, s);
 }
 
 arbx_status arbx_query_knn(arbx_handle h, const float* qpoints, int64_t nq, int k, int32_t* indices,

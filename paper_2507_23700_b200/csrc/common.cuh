@@ -121,9 +121,16 @@ arbx_status build_index(const float* prims, int64_t n, int dim, int kind, cudaSt
 arbx_status validate_index(const Index* ix, int64_t* violations_host, cudaStream_t s);
 
 // query_dN.cu (one TU per dimension), dispatched from query.cu
-using spatial_fn = arbx_status (*)(const Index*, const float* queries, int64_t nq, int qkind,
-                                   const uint32_t* qorder, int32_t* counts,
-                                   const int32_t* offsets, int32_t* indices, cudaStream_t);
+// One spatial traversal pass.  pass 0: counts[q] = matches.  pass 2: the same, and the first
+// `cap` matches of query q are stored in rows[q*cap ..]; *overflow counts the queries with
+// more than cap matches.  pass 1: fill indices[offsets[q] ..]; with cap > 0 only the queries
+// whose counts[q] > cap are traversed (the others are copied from rows by compact_rows).
+struct SpatialArgs {
+  const float* queries; int64_t nq; int qkind; const uint32_t* qorder;
+  int32_t* counts; const int32_t* offsets; int32_t* indices;
+  int32_t* rows; int cap; int* overflow; int pass;
+};
+using spatial_fn = arbx_status (*)(const Index*, const SpatialArgs&, cudaStream_t);
 using knn_fn = arbx_status (*)(const Index*, const float* qpoints, int64_t nq, int k,
                                const uint32_t* qorder, int32_t* indices, float* distances,
                                cudaStream_t);
@@ -135,5 +142,8 @@ const DimTable* dim_table(int dim);
 // scan.cu: offsets[0..nq] = exclusive scan of counts[0..nq); *total (device, int64) = sum
 arbx_status exclusive_scan_i32(const int32_t* counts, int32_t* offsets, int64_t nq,
                                long long* total_dev, cudaStream_t s);
+// scan.cu: indices[offsets[q] + j] = rows[q*cap + j] for j < counts[q], for every q with counts[q] <= cap
+arbx_status compact_rows(const int32_t* rows, int cap, const int32_t* counts, const int32_t* offsets,
+                         int32_t* indices, int64_t nq, cudaStream_t s);
 
 }  // namespace arbx

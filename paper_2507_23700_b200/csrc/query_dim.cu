@@ -146,7 +146,7 @@ __device__ __forceinline__ bool hits_prim(const Query<QK>& q, const float* p) {
 template <int PK, int QK, bool FILL>
 __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes, const float4* __restrict__ leaves,
                                                const int32_t* __restrict__ root, const Query<QK>& q,
-                                               int32_t* __restrict__ out) {
+                                               int32_t* __restrict__ out, int limit) {
   int cnt = 0;
   int32_t stack[STACK_DEPTH];
   int sp = 0;
@@ -173,7 +173,7 @@ __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes,
       Leaf<PK> lf;
       load_leaf<PK>(leaves, j, lf);
       if (hits_prim<QK, PK>(q, lf.v)) {
-        if constexpr (FILL) out[cnt] = (int32_t)(lf.idx & ~LEAF_END);
+        if constexpr (FILL) { if (cnt < limit) out[cnt] = (int32_t)(lf.idx & ~LEAF_END); }
         ++cnt;
       }
       if (lf.idx & LEAF_END) break;
@@ -223,7 +223,10 @@ __device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, in
   nd.l = __float_as_int(t.z); nd.r = __float_as_int(t.w);
 }
 
-template <int PK, int QK, bool FILL>
+// MODE 0: count.  MODE 1: fill the CSR slices (offsets known); with cap > 0 the queries whose
+// count is <= cap are skipped (their rows were stored by MODE 2 and are copied by
+// compact_rows).  MODE 2: count AND store the first `cap` hits of query q in rows[q*cap ..].
+template <int PK, int QK, int MODE>
 __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ nodes,
                                                      const float4* __restrict__ leaves,
                                                      const int32_t* __restrict__ root, int n,
@@ -231,26 +234,43 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
                                                      const uint32_t* __restrict__ qorder, int64_t nq,
                                                      int32_t* __restrict__ counts,
                                                      const int32_t* __restrict__ offsets,
-                                                     int32_t* __restrict__ indices, int mode, float alpha) {
+                                                     int32_t* __restrict__ indices, int cap,
+                                                     int* __restrict__ overflow, int mode, float alpha) {
+  constexpr bool FILL = MODE != 0;     // hits are written somewhere
   constexpr int QW = prim_width(QK, D);
   __shared__ int32_t s_stack[QT / 32][STACK_DEPTH];
   int32_t* stack = s_stack[threadIdx.x >> 5];
   const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
   const bool valid = t < nq;
   const int64_t qi = valid ? (qorder ? (int64_t)qorder[t] : t) : 0;
+  bool alive = valid;
+  if constexpr (MODE == 1) {   // rows that were stored are copied, not traversed again
+    if (cap > 0) {
+      alive = alive && counts[qi] > cap;
+      if (!__any_sync(~0u, alive)) return;
+    }
+  }
   Query<QK> q;
 #pragma unroll
   for (int e = 0; e < QW; ++e) q.v[e] = __ldg(queries + qi * QW + e);
-  bool alive = valid;
   if constexpr (QK == KIND_SPHERE) {
     q.r2 = q.v[D] * q.v[D];
     alive = alive && q.v[D] >= 0.f;      // negative radius matches nothing (reading A21)
   }
+  int64_t base64 = 0;   // where this query's hits go in `indices` (MODE 1: CSR slice, MODE 2: row q*cap)
+  int limit = INT32_MAX;
+  if constexpr (MODE == 1) {
+    base64 = valid ? offsets[qi] : 0;
+  }
+  if constexpr (MODE == 2) { base64 = qi * cap; limit = cap; }
   // mode 0: per-warp choice; 1: always one query per lane; 2: always packet
   if (mode == 1 || (mode == 0 && !warp_coherent<QK>(q, valid, alpha))) {
     int c = 0;
-    if (alive) c = thread_traverse<PK, QK, FILL>(nodes, leaves, root, q, FILL ? indices + offsets[qi] : nullptr);
-    if constexpr (!FILL) { if (valid) counts[qi] = c; }
+    if (alive) c = thread_traverse<PK, QK, FILL>(nodes, leaves, root, q, FILL ? indices + base64 : nullptr, limit);
+    if constexpr (MODE != 1) {
+      if (valid) counts[qi] = c;
+      if constexpr (MODE == 2) { if (c > cap) atomicAdd(overflow, 1); }
+    }
     return;
   }
   // FILL: hits are staged per lane in shared memory (FS slots, column `lane` of a padded
@@ -260,8 +280,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   __shared__ int32_t s_stage[FILL ? QT / 32 : 1][FILL ? FS * 33 : 1];
   int32_t* stage = s_stage[FILL ? (threadIdx.x >> 5) : 0];
   const int lane = threadIdx.x & 31;
-  int base = 0;      // FILL: position in `indices` of this query's next unflushed hit
-  if constexpr (FILL) base = valid ? offsets[qi] : 0;
+  int64_t base = base64;   // FILL: position in `indices` of this query's next unflushed hit
   int cnt = 0, pend = 0;
 
   auto flush = [&](uint32_t who) {   // who: lanes whose pending hits are written out (warp-uniform)
@@ -270,7 +289,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
       const int L = __ffs(who) - 1;
       who &= who - 1;
       const int m = __shfl_sync(~0u, pend, L);
-      const int b = __shfl_sync(~0u, base, L);
+      const int64_t b = __shfl_sync(~0u, base, L);
       if (lane < m) indices[b + lane] = stage[lane * 33 + L];
       if (lane == L) { base += pend; pend = 0; }
     }
@@ -288,7 +307,10 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
         for (int j = j0; j < je; ++j) {
           Leaf<PK> lf;
           load_leaf<PK>(leaves, first + j, lf);
-          if (alive && hits_prim<QK, PK>(q, lf.v)) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
+          if (alive && hits_prim<QK, PK>(q, lf.v)) {
+            if (MODE == 1 || cnt < limit) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
+            ++cnt;
+          }
         }
       }
     } else {
@@ -327,8 +349,11 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
       }
     }
   }
-  if constexpr (FILL) { flush(__ballot_sync(~0u, pend > 0)); }
-  else { if (valid) counts[qi] = cnt; }
+  if constexpr (FILL) flush(__ballot_sync(~0u, pend > 0));
+  if constexpr (MODE != 1) {
+    if (valid) counts[qi] = cnt;
+    if constexpr (MODE == 2) { if (cnt > cap) atomicAdd(overflow, 1); }
+  }
 }
 
 // ---- K1 / K2: k nearest neighbours ------------------------------------------------------------------
@@ -633,39 +658,39 @@ inline int traversal_mode() {
 
 // ---- host dispatch ------------------------------------------------------------------------------------
 template <int PK, int QK>
-arbx_status spatial_launch(const Index* ix, const float* queries, int64_t nq, const uint32_t* qorder,
-                           int32_t* counts, const int32_t* offsets, int32_t* indices, cudaStream_t s) {
-  const unsigned grid = (unsigned)((nq + QT - 1) / QT);
+arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s) {
+  const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);
   const float4* nodes = reinterpret_cast<const float4*>(ix->nodes);
   const float4* leaves = reinterpret_cast<const float4*>(ix->leaves);
-  ProfScope ps(indices ? K_SPATIAL_FILL : K_SPATIAL_COUNT, s);
+  ProfScope ps(a.pass == 1 ? K_SPATIAL_FILL : K_SPATIAL_COUNT, s);
   const int mode = traversal_mode();
   float alpha = 0.75f;
   if (const char* v = getenv("ARBX_PACKET_ALPHA")) alpha = (float)atof(v);
-  if (indices)
-    spatial_kernel<PK, QK, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices, mode, alpha);
+  const int n = (int)ix->n;
+  if (a.pass == 1)
+    spatial_kernel<PK, QK, 1><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, mode, alpha);
+  else if (a.pass == 2)
+    spatial_kernel<PK, QK, 2><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, mode, alpha);
   else
-    spatial_kernel<PK, QK, false><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, (int)ix->n, queries, qorder, nq, counts, offsets, indices, mode, alpha);
+    spatial_kernel<PK, QK, 0><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, 0, nullptr, mode, alpha);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
 
 template <int PK>
-arbx_status spatial_pk(const Index* ix, const float* queries, int64_t nq, int qkind, const uint32_t* qorder,
-                       int32_t* counts, const int32_t* offsets, int32_t* indices, cudaStream_t s) {
-  switch (qkind) {
-    case KIND_POINT: return spatial_launch<PK, KIND_POINT>(ix, queries, nq, qorder, counts, offsets, indices, s);
-    case KIND_BOX: return spatial_launch<PK, KIND_BOX>(ix, queries, nq, qorder, counts, offsets, indices, s);
-    default: return spatial_launch<PK, KIND_SPHERE>(ix, queries, nq, qorder, counts, offsets, indices, s);
+arbx_status spatial_pk(const Index* ix, const SpatialArgs& a, cudaStream_t s) {
+  switch (a.qkind) {
+    case KIND_POINT: return spatial_launch<PK, KIND_POINT>(ix, a, s);
+    case KIND_BOX: return spatial_launch<PK, KIND_BOX>(ix, a, s);
+    default: return spatial_launch<PK, KIND_SPHERE>(ix, a, s);
   }
 }
 
-arbx_status spatial_entry(const Index* ix, const float* queries, int64_t nq, int qkind, const uint32_t* qorder,
-                          int32_t* counts, const int32_t* offsets, int32_t* indices, cudaStream_t s) {
+arbx_status spatial_entry(const Index* ix, const SpatialArgs& a, cudaStream_t s) {
   switch (ix->kind) {
-    case KIND_POINT: return spatial_pk<KIND_POINT>(ix, queries, nq, qkind, qorder, counts, offsets, indices, s);
-    case KIND_BOX: return spatial_pk<KIND_BOX>(ix, queries, nq, qkind, qorder, counts, offsets, indices, s);
-    default: return spatial_pk<KIND_SPHERE>(ix, queries, nq, qkind, qorder, counts, offsets, indices, s);
+    case KIND_POINT: return spatial_pk<KIND_POINT>(ix, a, s);
+    case KIND_BOX: return spatial_pk<KIND_BOX>(ix, a, s);
+    default: return spatial_pk<KIND_SPHERE>(ix, a, s);
   }
 }
 

@@ -77,7 +77,36 @@ __global__ void __launch_bounds__(ST) apply_kernel(const int32_t* __restrict__ c
 
 __global__ void zero_total_kernel(int32_t* offsets, long long* total) { offsets[0] = 0; *total = 0; }
 
+// A warp copies the stored rows of 32 consecutive queries into their (adjacent) CSR slices.
+__global__ void __launch_bounds__(ST) compact_rows_kernel(const int32_t* __restrict__ rows, int cap,
+                                                          const int32_t* __restrict__ counts,
+                                                          const int32_t* __restrict__ offsets,
+                                                          int32_t* __restrict__ indices, int64_t nq) {
+  const int lane = threadIdx.x & 31;
+  const int64_t q0 = ((int64_t)blockIdx.x * ST + threadIdx.x) - lane;   // first query of this warp
+  if (q0 >= nq) return;
+  const int64_t q = q0 + lane;
+  const int c = q < nq ? counts[q] : 0;
+  const int o = q < nq ? offsets[q] : 0;
+  for (int L = 0; L < 32; ++L) {
+    const int cl = __shfl_sync(~0u, c, L);
+    const int ol = __shfl_sync(~0u, o, L);
+    if (cl > cap) continue;                       // filled by the traversal pass instead
+    const int32_t* row = rows + (q0 + L) * cap;
+    for (int j = lane; j < cl; j += 32) indices[ol + j] = row[j];
+  }
+}
+
 }  // namespace
+
+arbx_status compact_rows(const int32_t* rows, int cap, const int32_t* counts, const int32_t* offsets,
+                         int32_t* indices, int64_t nq, cudaStream_t s) {
+  if (nq == 0) return ARBX_OK;
+  ProfScope ps(K_SPATIAL_FILL, s);
+  compact_rows_kernel<<<(unsigned)((nq + ST - 1) / ST), ST, 0, s>>>(rows, cap, counts, offsets, indices, nq);
+  ARBX_LAUNCH_CHECK();
+  return ARBX_OK;
+}
 
 arbx_status exclusive_scan_i32(const int32_t* counts, int32_t* offsets, int64_t nq, long long* total_dev,
                                cudaStream_t s) {
