@@ -88,6 +88,7 @@ __global__ void __launch_bounds__(ST) compact_rows_kernel(const int32_t* __restr
   const int64_t q = q0 + lane;
   const int c = q < nq ? counts[q] : 0;
   const int o = q < nq ? offsets[q] : 0;
+#pragma unroll 8
   for (int L = 0; L < 32; ++L) {
     const int cl = __shfl_sync(~0u, c, L);
     const int ol = __shfl_sync(~0u, o, L);

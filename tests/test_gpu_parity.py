@@ -350,3 +350,42 @@ def _sampled_full(arbx, orc, name, nsample=2000):
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
 def test_configs_full_sampled(arbx, orc, name):
     _sampled_full(arbx, orc, name)
+
+
+# ---- every traversal / CSR-assembly path gives the same answer ------------------------------------------
+@pytest.mark.parametrize("traversal", ["thread", "packet", None])
+@pytest.mark.parametrize("budget_mb", ["0", "1", None])
+def test_paths_agree_with_oracle(arbx, orc, monkeypatch, traversal, budget_mb):
+    """ARBX_TRAVERSAL forces per-lane or packet traversal (default: per-warp choice);
+    ARBX_STORE_BUDGET_MB=0 forces count -> scan -> fill (two traversals), 1 MB gives 16-slot
+    stored rows so that dense queries overflow and take the second traversal."""
+    from oracle import compare as cmp
+    if traversal:
+        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    if budget_mb is not None:
+        monkeypatch.setenv("ARBX_STORE_BUDGET_MB", budget_mb)
+    prims = dg.uniform_points(6000, 3, 41)
+    qp = dg.uniform_points(4000, 3, 42)
+    q = dg.sphere_queries(qp, 0.09)          # ~18 hits per query on average: rows above and below 16
+    q[::7, 3] = 0.25                          # some very dense rows (hundreds of hits)
+    st = _spatial_case(arbx, orc, cmp, prims, dg.POINT, q, dg.SPHERE, f"paths {traversal} {budget_mb}")
+    assert st["pairs"] > 16 * 4000
+    boxes = dg.uniform_boxes(5000, 3, 43, 0.02)
+    qb = dg.uniform_boxes(3000, 3, 44, 0.05)
+    _spatial_case(arbx, orc, cmp, boxes, dg.BOX, qb, dg.BOX, f"paths boxes {traversal} {budget_mb}")
+    ix = arbx.Index(_dev(prims), dg.POINT)
+    for k in (3, 16, 33):
+        gi, gd = ix.query_knn(_dev(qp), k)
+        cmp.compare_knn(prims, dg.POINT, qp, k, orc.knn(prims, dg.POINT, qp, k), (_np(gi), _np(gd)), what=f"knn {traversal} k={k}")
+    ix.close()
+
+
+def test_coherent_and_scattered_warps_in_one_batch(arbx, orc):
+    """Half of the queries sit in one tight cluster (packet warps), half are spread out with tiny
+    radii (per-lane warps): the per-warp choice must not change any row."""
+    from oracle import compare as cmp
+    prims = dg.uniform_points(20000, 3, 51)
+    tight = (0.5 + 0.01 * dg.uniform_points(2048, 3, 52)).astype(np.float32)
+    loose = dg.uniform_points(2048, 3, 53)
+    q = np.concatenate([dg.sphere_queries(tight, 0.08), dg.sphere_queries(loose, 0.004)], axis=0)
+    _spatial_case(arbx, orc, cmp, prims, dg.POINT, q, dg.SPHERE, "mixed coherence")
