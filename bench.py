@@ -87,11 +87,37 @@ def algorithmic_bytes(cfg, totals):
     b["Q2_qsort_pass"] = nbatches * ((4 + 8) * nq + (qpass - 1) * 16 * nq)
     # traversal: order 4 + query row + result; the tree is read once per traversal
     per_count = nq * (4 + 4 * qw + 4) + tree
-    b["T1_spatial_count"] = 2 * per_count                       # once in _spatial, once in _count
-    b["T3_spatial_fill"] = nq * (4 + 4 * qw + 4) + 4 * pairs + tree
+    # arbx_query_count: one count traversal; arbx_query_spatial: one traversal that also stores
+    # the hits in scratch rows (both under the T1 id), then the rows are copied into the CSR
+    # slices (T3 id: rows read + indices written + counts and offsets read)
+    b["T1_spatial_count"] = per_count + (per_count + 4 * pairs)
+    b["T3_spatial_fill"] = 4 * pairs + 4 * pairs + 8 * nq
     if cfg["k"]:
         b["K1K2_knn"] = nq * (4 + 4 * D + 8 * cfg["k"]) + tree
     return b
+
+
+# kernel id -> substring of the CUDA kernel name in the committed ncu launch list
+_NCU_KERNEL = {"K1K2_knn": "knn_thread_kernel", "T1_spatial_count": "spatial_kernel", "T3_spatial_fill": "compact_rows",
+               "B5B6_hierarchy_refit": "hierarchy_kernel", "B3_sort_pass": "onesweep_pass<unsigned long long",
+               "Q2_qsort_pass": "onesweep_pass<unsigned int"}
+
+
+def ncu_traffic(kernel_id: str, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    committed ncu capture of this same workload (profiles/r1_launches_C3.csv); None if absent."""
+    path = os.path.join(ROOT, "profiles", f"r1_launches_{workload}.csv")
+    pat = _NCU_KERNEL.get(kernel_id)
+    if not pat or not os.path.exists(path):
+        return None
+    import csv
+    tot, cnt = 0.0, 0
+    with open(path) as f:
+        for r in csv.DictReader(f):
+            if pat in r["kernel"]:
+                tot += float(r["dram_read_bytes"]) + float(r["dram_write_bytes"])
+                cnt += 1
+    return int(tot / cnt) if cnt else None
 
 
 def max_over_ranks(vals, device=None):
@@ -393,7 +419,7 @@ def main():
         # per-LAUNCH figures for the dominant kernel
         lps = max(dk["launches_per_step"], 1)
         roofline = dict(bound="hbm", kernel=dom, achieved=dk["achieved_gbs"], peak=peak, unit="GB/s",
-                        frac=dk["frac_of_peak"], traffic=None, peak_source=peak_src,
+                        frac=dk["frac_of_peak"], traffic=ncu_traffic(dom, cfg["name"]), peak_source=peak_src,
                         algorithmic_bytes_per_launch=int(ab[dom] / lps) if ab.get(dom) else None,
                         ms_per_launch=round(dk["ms_per_step"] / lps, 4), share_of_step=dk["share"])
         build_bytes = sum(ab[x] for x in ab if x.startswith("B"))

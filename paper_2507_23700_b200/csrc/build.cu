@@ -219,25 +219,31 @@ hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict
     float* node = nodes + (int64_t)p * NW;
     const int slot = left_child ? 0 : 1;
     const int sib = 1 - slot;
+    auto store_half = [&]() {   // this child's box and reference, for the traversal kernels
 #pragma unroll
-    for (int a = 0; a < D; ++a) {
-      __stcg(node + slot * 2 * D + a, lo[a]);
-      __stcg(node + slot * 2 * D + D + a, hi[a]);
-    }
-    __stcg(reinterpret_cast<int*>(node) + 4 * D + slot, ref);
+      for (int a = 0; a < D; ++a) {
+        __stcg(node + slot * 2 * D + a, lo[a]);
+        __stcg(node + slot * 2 * D + D + a, hi[a]);
+      }
+      __stcg(reinterpret_cast<int*>(node) + 4 * D + slot, ref);
+    };
     int other;
     if (local) {
+      // the sibling reads our box from shared memory, so the global stores stay outside the
+      // fence -> atomic window (a fence would otherwise wait for them)
       float* mine = s_box[slot][p - c0];
 #pragma unroll
       for (int a = 0; a < D; ++a) { mine[a] = lo[a]; mine[D + a] = hi[a]; }
       __threadfence_block();
       other = atomicExch(&s_flag[p - c0], left_child ? l : r);
+      store_half();
       if (other == -1) return;   // first to arrive: the sibling's thread carries on
       __threadfence_block();
       const volatile float* theirs = s_box[sib][p - c0];
 #pragma unroll
       for (int a = 0; a < D; ++a) { lo[a] = fminf(lo[a], theirs[a]); hi[a] = fmaxf(hi[a], theirs[D + a]); }
     } else {
+      store_half();
       __threadfence();
       other = atomicExch(flags + p, left_child ? l : r);
       if (other == -1) return;
