@@ -94,6 +94,14 @@ ARBX_API arbx_status arbx_bounds(arbx_handle h, float* lo_host, float* hi_host, 
 ARBX_API arbx_status arbx_query_count(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
                              int32_t* counts, arbx_stream stream);
 
+/* Capped count = the pure-callback query whose callback stops a query's traversal once it
+ * has seen `limit` matches (PAPER.md:L174 CallbackTreeTraversalControl::early_exit; L180-209
+ * the CountUpToN example; L306).  counts[q] = min(matches of query q, limit), limit >= 1.
+ * Reading A20: the paper's example post-increments and therefore stores
+ * min(total, n+1); this call returns min(total, limit).  Other arguments as arbx_query_count. */
+ARBX_API arbx_status arbx_query_count_upto(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                                  int32_t limit, int32_t* counts, arbx_stream stream);
+
 /* Storage search (PAPER.md:L69 v1 "indices and offsets"; L112-115 overload 3).
  * offsets: DEVICE int32[nq+1]; offsets[0]=0, offsets[q+1]-offsets[q] = matches of query q,
  * offsets[nq] = total.  indices: DEVICE int32[indices_capacity] or NULL; the slice

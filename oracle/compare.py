@@ -107,3 +107,19 @@ def compare_knn(prims, pkind: int, qpoints, k: int, orc, got, eps: float = EPS, 
             f"{what}: distance mismatch, max rel {np.max(np.abs(gd - od) / np.maximum(od, 1e-300)):.3e}")
         # (4) the reported distance belongs to the reported index
         assert np.all(np.abs(gd - d_true) <= eps * d_true + abs_tol), f"{what}: distance does not match its index"
+
+
+def compare_counts_upto(orc, counts, limit: int, what: str = "") -> None:
+    """Capped count (PAPER.md:L180-209 CountUpToN, reading A20): the definition is
+    min(|row(q)|, limit); with the tolerance band, min(|sure|, limit) <= counts[q] <=
+    min(|sure| + |band|, limit)."""
+    o_off, _, o_band = orc
+    o_off = np.asarray(o_off, dtype=np.int64)
+    allc = np.diff(o_off)
+    bandc = np.add.reduceat(np.concatenate([np.asarray(o_band, dtype=np.int64), [0]]),
+                            np.minimum(o_off[:-1], len(o_band)))
+    bandc = np.where(allc == 0, 0, bandc)
+    counts = np.asarray(counts, dtype=np.int64)
+    lo, hi = np.minimum(allc - bandc, limit), np.minimum(allc, limit)
+    bad = (counts < lo) | (counts > hi)
+    assert not bad.any(), f"{what}: {int(bad.sum())} capped counts outside [min(sure,L), min(sure+band,L)], first q={int(np.argmax(bad))}"

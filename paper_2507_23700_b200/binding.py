@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libarbx.so")
 
 EXPORTS = (
     "arbx_build", "arbx_destroy", "arbx_size", "arbx_bounds", "arbx_query_count",
-    "arbx_query_spatial", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
+    "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
     "arbx_launch_count", "arbx_profile_enable", "arbx_profile_num_kernels",
     "arbx_profile_kernel_name", "arbx_profile_read", "arbx_status_string", "arbx_last_error",
 )
@@ -54,6 +54,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_size.argtypes = [vp, ctypes.POINTER(i64)]
         L.arbx_bounds.argtypes = [vp, vp, vp, vp]
         L.arbx_query_count.argtypes = [vp, vp, i64, i32, vp, vp]
+        L.arbx_query_count_upto.argtypes = [vp, vp, i64, i32, i32, vp, vp]
         L.arbx_query_spatial.argtypes = [vp, vp, i64, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.arbx_query_knn.argtypes = [vp, vp, i64, i32, vp, vp, vp]
         L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
@@ -69,7 +70,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_status_string.restype = ctypes.c_char_p
         L.arbx_status_string.argtypes = [i32]
         L.arbx_last_error.restype = ctypes.c_char_p
-        for name in EXPORTS[:9]:
+        for name in EXPORTS[:10]:
             getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -132,6 +133,12 @@ def arbx_query_count(handle: int, queries: torch.Tensor, nq: int, qkind: int, co
                      stream=None) -> None:
     _check(lib().arbx_query_count(handle, _ptr(queries), nq, qkind, _ptr(counts), _stream(stream)),
            "arbx_query_count")
+
+
+def arbx_query_count_upto(handle: int, queries: torch.Tensor, nq: int, qkind: int, limit: int,
+                          counts: torch.Tensor, stream=None) -> None:
+    _check(lib().arbx_query_count_upto(handle, _ptr(queries), nq, qkind, limit, _ptr(counts), _stream(stream)),
+           "arbx_query_count_upto")
 
 
 def arbx_query_spatial(handle: int, queries: torch.Tensor, nq: int, qkind: int, offsets: torch.Tensor,
@@ -221,10 +228,15 @@ class Index:
         _dev_f32(queries, "queries")
         return queries.numel() // row_width(qkind, self.dim)
 
-    def query_count(self, queries: torch.Tensor, qkind: int = SPHERE, stream=None) -> torch.Tensor:
+    def query_count(self, queries: torch.Tensor, qkind: int = SPHERE, stream=None,
+                    limit: int | None = None) -> torch.Tensor:
+        """counts[q] = matches of query q; with `limit`, min(matches, limit) with early exit."""
         nq = self._nq(queries, qkind)
         counts = torch.empty(nq, dtype=torch.int32, device=self.device)
-        arbx_query_count(self.handle, queries, nq, qkind, counts, stream)
+        if limit is None:
+            arbx_query_count(self.handle, queries, nq, qkind, counts, stream)
+        else:
+            arbx_query_count_upto(self.handle, queries, nq, qkind, limit, counts, stream)
         return counts
 
     def query_spatial(self, queries: torch.Tensor, qkind: int = SPHERE, capacity: int | None = None,

@@ -187,8 +187,22 @@ arbx_status arbx_bounds(arbx_handle h, float* lo_host, float* hi_host, arbx_stre
   return ARBX_OK;
 }
 
+static arbx_status count_impl(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                              int32_t limit, int32_t* counts, arbx_stream stream);
+
 arbx_status arbx_query_count(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
                              int32_t* counts, arbx_stream stream) {
+  return count_impl(h, queries, nq, qkind, 0, counts, stream);
+}
+
+arbx_status arbx_query_count_upto(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                                  int32_t limit, int32_t* counts, arbx_stream stream) {
+  if (limit < 1) { set_error("arbx_query_count_upto: limit must be >= 1"); return ARBX_ERR_INVALID_ARG; }
+  return count_impl(h, queries, nq, qkind, limit, counts, stream);
+}
+
+static arbx_status count_impl(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                              int32_t limit, int32_t* counts, arbx_stream stream) {
   if (!h || nq < 0 || bad_kind((int)qkind) || (nq > 0 && (!queries || !counts))) {
     set_error("arbx_query_count: invalid argument");
     return ARBX_ERR_INVALID_ARG;
@@ -200,7 +214,7 @@ arbx_status arbx_query_count(arbx_handle h, const float* queries, int64_t nq, ar
   if (ix->n == 0) { ARBX_CUDA(cudaMemsetAsync(counts, 0, (size_t)nq * sizeof(int32_t), s)); return ARBX_OK; }
   Scratch<uint32_t> order;
   ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
-  SpatialArgs a{queries, nq, (int)qkind, order.p, counts, nullptr, nullptr, nullptr, 0, nullptr, 0};
+  SpatialArgs a{queries, nq, (int)qkind, order.p, counts, nullptr, nullptr, nullptr, limit, nullptr, 0};
   return dim_table(ix->dim)->spatial(ix, a, s);
 }
 

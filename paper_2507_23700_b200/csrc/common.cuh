@@ -121,7 +121,8 @@ arbx_status build_index(const float* prims, int64_t n, int dim, int kind, cudaSt
 arbx_status validate_index(const Index* ix, int64_t* violations_host, cudaStream_t s);
 
 // query_dN.cu (one TU per dimension), dispatched from query.cu
-// One spatial traversal pass.  pass 0: counts[q] = matches.  pass 2: the same, and the first
+// One spatial traversal pass.  pass 0: counts[q] = matches (cap > 0: min(matches, cap), with
+// early exit).  pass 2: the same, and the first
 // `cap` matches of query q are stored in rows[q*cap ..]; *overflow counts the queries with
 // more than cap matches.  pass 1: fill indices[offsets[q] ..]; with cap > 0 only the queries
 // whose counts[q] > cap are traversed (the others are copied from rows by compact_rows).

@@ -175,6 +175,7 @@ __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes,
       if (hits_prim<QK, PK>(q, lf.v)) {
         if constexpr (FILL) { if (cnt < limit) out[cnt] = (int32_t)(lf.idx & ~LEAF_END); }
         ++cnt;
+        if constexpr (!FILL) { if (cnt >= limit) return cnt; }   // capped count: early exit
       }
       if (lf.idx & LEAF_END) break;
     }
@@ -263,6 +264,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
     base64 = valid ? offsets[qi] : 0;
   }
   if constexpr (MODE == 2) { base64 = qi * cap; limit = cap; }
+  if constexpr (MODE == 0) { if (cap > 0) limit = cap; }   // capped count (arbx_query_count_upto)
   // mode 0: per-warp choice; 1: always one query per lane; 2: always packet
   if (mode == 1 || (mode == 0 && !warp_coherent<QK>(q, valid, alpha))) {
     int c = 0;
@@ -320,6 +322,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
         load_leaf<PK>(leaves, first + j, lf);
         cnt += (alive && hits_prim<QK, PK>(q, lf.v)) ? 1 : 0;
       }
+      if (cnt >= limit) alive = false;   // capped count: this lane has seen enough
     }
   };
 
@@ -336,6 +339,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
         const bool a1 = __any_sync(~0u, alive && hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D));
         if (a0 && nd.c0 < 0) leaf_range(nd.l, ref - nd.l + 1);
         if (a1 && nd.c1 < 0) leaf_range(ref + 1, nd.r - ref);
+        if constexpr (MODE == 0) { if (cap > 0 && !__any_sync(~0u, alive)) break; }
         const bool in0 = a0 && nd.c0 >= 0, in1 = a1 && nd.c1 >= 0;
         if (in0) {
           ref = nd.c0;
@@ -351,7 +355,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   }
   if constexpr (FILL) flush(__ballot_sync(~0u, pend > 0));
   if constexpr (MODE != 1) {
-    if (valid) counts[qi] = cnt;
+    if (valid) counts[qi] = MODE == 0 ? min(cnt, limit) : cnt;
     if constexpr (MODE == 2) { if (cnt > cap) atomicAdd(overflow, 1); }
   }
 }
@@ -672,7 +676,7 @@ arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s
   else if (a.pass == 2)
     spatial_kernel<PK, QK, 2><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, mode, alpha);
   else
-    spatial_kernel<PK, QK, 0><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, 0, nullptr, mode, alpha);
+    spatial_kernel<PK, QK, 0><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, a.cap, nullptr, mode, alpha);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }

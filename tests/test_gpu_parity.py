@@ -389,3 +389,42 @@ def test_coherent_and_scattered_warps_in_one_batch(arbx, orc):
     loose = dg.uniform_points(2048, 3, 53)
     q = np.concatenate([dg.sphere_queries(tight, 0.08), dg.sphere_queries(loose, 0.004)], axis=0)
     _spatial_case(arbx, orc, cmp, prims, dg.POINT, q, dg.SPHERE, "mixed coherence")
+
+
+# ---- NEXT-1: capped count with early exit ----------------------------------------
+@pytest.mark.parametrize("traversal", ["thread", "packet", None])
+def test_count_upto(arbx, orc, monkeypatch, traversal):
+    from oracle import compare as cmp
+    if traversal:
+        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    prims = dg.uniform_points(8000, 3, 61)
+    q = dg.sphere_queries(dg.uniform_points(5000, 3, 62), 0.08)
+    o = orc.spatial(prims, dg.POINT, q, dg.SPHERE)
+    ix = arbx.Index(_dev(prims), dg.POINT)
+    full = _np(ix.query_count(_dev(q), dg.SPHERE))
+    for limit in (1, 5, 17, 10_000):
+        c = _np(ix.query_count(_dev(q), dg.SPHERE, limit=limit))
+        cmp.compare_counts_upto(o, c, limit, f"upto {limit} {traversal}")
+        assert np.array_equal(c, np.minimum(full, limit))      # same arithmetic as the uncapped count
+    with pytest.raises(arbx.ArbxError):
+        ix.query_count(_dev(q), dg.SPHERE, limit=0)
+    ix.close()
+    # exact predicate (boxes): bit-exact against the definition min(|row|, limit)
+    boxes = dg.uniform_boxes(6000, 3, 63, 0.03)
+    qb = dg.uniform_boxes(3000, 3, 64, 0.05)
+    ob = orc.spatial(boxes, dg.BOX, qb, dg.BOX)
+    ixb = arbx.Index(_dev(boxes), dg.BOX)
+    for limit in (2, 9):
+        c = _np(ixb.query_count(_dev(qb), dg.BOX, limit=limit))
+        assert np.array_equal(c, np.minimum(np.diff(ob[0]), limit))
+    ixb.close()
+
+
+def test_count_upto_lattice_closed_form(arbx):
+    p = dg.lattice_points(8, 3)
+    ix = arbx.Index(_dev(p), dg.POINT)
+    expect = 1 + (p > 0).sum(1) + (p < 7).sum(1)             # r = 1: self + in-range axis neighbours
+    for limit in (1, 4, 7, 50):
+        c = _np(ix.query_count(_dev(dg.sphere_queries(p, 1.0)), dg.SPHERE, limit=limit))
+        assert np.array_equal(c, np.minimum(expect, limit))
+    ix.close()

@@ -267,3 +267,18 @@ def test_sphere_primitive_knn_distance(orc):
     b = np.array([[0, 0, 0, 1, 1, 1]], dtype=np.float32)
     _, d = orc.knn(b, dg.BOX, np.array([[0.5, 0.5, 0.5], [2, 2, 1]], dtype=np.float32), 1)
     assert d[0, 0] == 0.0 and np.isclose(d[1, 0], np.sqrt(2.0))
+
+
+def test_capped_count_comparator_is_min_of_definition(orc):
+    """compare_counts_upto accepts exactly min(|row|, limit) on an exact-predicate case and
+    rejects an off-by-one (the CountUpToN example's min(total, n+1), reading A20)."""
+    from oracle import compare as cmp
+    from paper_2507_23700_b200 import datagen as dg
+    cells = dg.lattice_cells(5, 2)
+    o = orc.spatial(cells, dg.BOX, cells, dg.BOX)
+    rows = np.diff(o[0])
+    assert rows.max() == 9 and rows.min() == 4                # 3^2 interior, 2^2 corners (touching counts)
+    for limit in (1, 4, 6, 20):
+        cmp.compare_counts_upto(o, np.minimum(rows, limit), limit)
+    with pytest.raises(AssertionError):
+        cmp.compare_counts_upto(o, np.minimum(rows, 6 + 1), 6)
