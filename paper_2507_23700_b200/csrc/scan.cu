@@ -77,7 +77,9 @@ __global__ void __launch_bounds__(ST) apply_kernel(const int32_t* __restrict__ c
 
 __global__ void zero_total_kernel(int32_t* offsets, long long* total) { offsets[0] = 0; *total = 0; }
 
-// A warp copies the stored rows of 32 consecutive queries into their (adjacent) CSR slices.
+// A warp copies the stored rows of 32 consecutive queries into their CSR slices, which are
+// adjacent: lane-strided over the ELEMENTS of the 32 slices (coalesced stores, independent
+// loads); the row of an element is found by a 5-step search over the warp's 32 offsets.
 __global__ void __launch_bounds__(ST) compact_rows_kernel(const int32_t* __restrict__ rows, int cap,
                                                           const int32_t* __restrict__ counts,
                                                           const int32_t* __restrict__ offsets,
@@ -86,15 +88,23 @@ __global__ void __launch_bounds__(ST) compact_rows_kernel(const int32_t* __restr
   const int64_t q0 = ((int64_t)blockIdx.x * ST + threadIdx.x) - lane;   // first query of this warp
   if (q0 >= nq) return;
   const int64_t q = q0 + lane;
+  const int64_t qend = q0 + 32 < nq ? q0 + 32 : nq;
+  const int o0 = offsets[q0];
+  const int T = offsets[qend] - o0;                 // elements in this warp's 32 slices
   const int c = q < nq ? counts[q] : 0;
-  const int o = q < nq ? offsets[q] : 0;
-#pragma unroll 8
-  for (int L = 0; L < 32; ++L) {
-    const int cl = __shfl_sync(~0u, c, L);
-    const int ol = __shfl_sync(~0u, o, L);
-    if (cl > cap) continue;                       // filled by the traversal pass instead
-    const int32_t* row = rows + (q0 + L) * cap;
-    for (int j = lane; j < cl; j += 32) indices[ol + j] = row[j];
+  const int rel = q < nq ? offsets[q] - o0 : T;     // start of lane's slice relative to the warp's
+#pragma unroll 2
+  for (int e0 = 0; e0 < T; e0 += 32) {
+    const int e = e0 + lane;
+    int row = 0;
+#pragma unroll
+    for (int step = 16; step > 0; step >>= 1) {
+      const int cand = row + step;                  // <= 31
+      if (__shfl_sync(~0u, rel, cand) <= e) row = cand;
+    }
+    const int cr = __shfl_sync(~0u, c, row);
+    const int rr = __shfl_sync(~0u, rel, row);
+    if (e < T && cr <= cap) indices[o0 + e] = rows[(q0 + row) * cap + (e - rr)];   // cr > cap: traversal pass
   }
 }
 
