@@ -210,6 +210,64 @@ __device__ __forceinline__ bool warp_coherent(const Query<QK>& q, bool valid, fl
   }
 }
 
+// Joint region of the (coherent) queries of a warp: the box [lo,hi] of the query centres /
+// query boxes and the largest radius.  joint_hits_prim is true whenever ANY lane's exact
+// hits_prim can be true (same monotone fp32 operation sequences), so it is used to discard
+// the primitives of a leaf range 32 at a time, one per lane, before the exact per-lane tests.
+template <int QK>
+struct Joint { float lo[D], hi[D]; float r, r2; };
+
+template <int QK>
+__device__ __forceinline__ void joint_of_warp(const Query<QK>& q, bool alive, Joint<QK>& J) {
+#pragma unroll
+  for (int a = 0; a < D; ++a) {
+    float lo = alive ? q.v[a] : INFINITY;
+    float hi = alive ? (QK == KIND_BOX ? q.v[D + a] : q.v[a]) : -INFINITY;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      lo = fminf(lo, __shfl_xor_sync(~0u, lo, o));
+      hi = fmaxf(hi, __shfl_xor_sync(~0u, hi, o));
+    }
+    J.lo[a] = lo; J.hi[a] = hi;
+  }
+  J.r = 0.f; J.r2 = 0.f;
+  if constexpr (QK == KIND_SPHERE) {
+    float r = alive ? q.v[D] : 0.f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) r = fmaxf(r, __shfl_xor_sync(~0u, r, o));
+    J.r = r; J.r2 = r * r;
+  }
+}
+
+template <int D_>
+__device__ __forceinline__ float dist2_bb(const float* alo, const float* ahi, const float* blo, const float* bhi) {
+  float s = 0.f;
+#pragma unroll
+  for (int a = 0; a < D_; ++a) {
+    float d = fmaxf(0.f, fmaxf(alo[a] - bhi[a], blo[a] - ahi[a]));
+    s = fmaf(d, d, s);
+  }
+  return s;
+}
+
+template <int QK, int PK>
+__device__ __forceinline__ bool joint_hits_prim(const Joint<QK>& J, const float* p) {
+  if constexpr (QK == KIND_SPHERE) {
+    if constexpr (PK == KIND_POINT) return dist2_pb<D>(p, J.lo, J.hi) <= J.r2;
+    else if constexpr (PK == KIND_BOX) return dist2_bb<D>(p, p + D, J.lo, J.hi) <= J.r2;
+    else { const float rr = J.r + p[D]; return dist2_pb<D>(p, J.lo, J.hi) <= rr * rr; }
+  } else {   // BOX queries: J is the union box
+    if constexpr (PK == KIND_SPHERE) {
+      return dist2_pb<D>(p, J.lo, J.hi) <= p[D] * p[D];
+    } else {
+      bool ok = true;
+#pragma unroll
+      for (int a = 0; a < D; ++a) ok = ok && p[a] <= J.hi[a] && J.lo[a] <= (PK == KIND_BOX ? p[D + a] : p[a]);
+      return ok;
+    }
+  }
+}
+
 struct NodeX { float v[4 * D]; int32_t c0, c1, l, r; };
 
 __device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, int32_t ref, NodeX& nd) {
@@ -298,32 +356,39 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
     __syncwarp();
   };
 
-  constexpr int CH = 4;     // FILL: staging room is checked once per CH primitives
+  // Leaf ranges: lane j first tests primitive j against the warp's JOINT region (one
+  // coalesced load, 32 primitives at a time); only the survivors are broadcast to all lanes
+  // for the exact per-lane test.
+  Joint<QK> J;
+  joint_of_warp<QK>(q, alive, J);
   auto leaf_range = [&](int first, int m) {   // m is warp-uniform
-    if constexpr (FILL) {
-      for (int j0 = 0; j0 < m; j0 += CH) {
-        const uint32_t full = __ballot_sync(~0u, pend > FS - CH);
-        if (full) flush(full);
-        const int je = min(m, j0 + CH);
-#pragma unroll 4
-        for (int j = j0; j < je; ++j) {
-          Leaf<PK> lf;
-          load_leaf<PK>(leaves, first + j, lf);
-          if (alive && hits_prim<QK, PK>(q, lf.v)) {
+    for (int j0 = 0; j0 < m; j0 += 32) {
+      bool in = false;
+      if (j0 + lane < m) {
+        Leaf<PK> mine;
+        load_leaf<PK>(leaves, first + j0 + lane, mine);
+        in = joint_hits_prim<QK, PK>(J, mine.v);
+      }
+      uint32_t todo = __ballot_sync(~0u, in);
+      while (todo) {
+        const int b = __ffs(todo) - 1;
+        todo &= todo - 1;
+        Leaf<PK> lf;
+        load_leaf<PK>(leaves, first + j0 + b, lf);
+        const bool hit = alive && hits_prim<QK, PK>(q, lf.v);
+        if constexpr (FILL) {
+          const uint32_t full = __ballot_sync(~0u, pend == FS);
+          if (full) flush(full);
+          if (hit) {
             if (MODE == 1 || cnt < limit) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
             ++cnt;
           }
+        } else {
+          cnt += hit ? 1 : 0;
         }
       }
-    } else {
-#pragma unroll 4
-      for (int j = 0; j < m; ++j) {
-        Leaf<PK> lf;
-        load_leaf<PK>(leaves, first + j, lf);
-        cnt += (alive && hits_prim<QK, PK>(q, lf.v)) ? 1 : 0;
-      }
-      if (cnt >= limit) alive = false;   // capped count: this lane has seen enough
     }
+    if constexpr (MODE == 0) { if (cnt >= limit) alive = false; }   // capped count: seen enough
   };
 
   if (__any_sync(~0u, alive)) {
