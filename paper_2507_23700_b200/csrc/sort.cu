@@ -14,12 +14,15 @@ namespace arbx {
 namespace {
 
 constexpr int RADIX = 256;
-constexpr int SORT_THREADS = 256;
+constexpr int SORT_THREADS = 512;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_IPT = 16;                         // items per thread
+constexpr int SORT_IPT = 8;                          // items per thread
 constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;   // 4096 elements per tile
 constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_INCL = 2u << 30, VAL_MASK = (1u << 30) - 1;
 constexpr int MAX_PASSES = 8;
+#ifndef SORT_LB
+#define SORT_LB 8
+#endif
 
 __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
   uint32_t v;
@@ -97,22 +100,24 @@ __global__ void __launch_bounds__(RADIX) hist_scan_kernel(uint32_t* ghist) {
 
 // ---- one digit pass ------------------------------------------------------------------------
 template <typename K, bool IOTA, bool VALS>
-__global__ void __launch_bounds__(SORT_THREADS)
+__global__ void __launch_bounds__(SORT_THREADS, 2)
 onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* __restrict__ vin,
               uint32_t* __restrict__ vout, uint32_t n, int shift,
               const uint32_t* __restrict__ digit_base, uint32_t* __restrict__ counter,
               uint32_t* __restrict__ status) {
-  __shared__ union { K keys[SORT_TILE]; uint32_t vals[SORT_TILE]; } sm;
-  __shared__ uint32_t whist[SORT_WARPS][RADIX];
+  // dynamic shared memory: the tile (keys, later reused for values) then the per-warp digit counters
+  extern __shared__ __align__(16) unsigned char sort_smem[];
+  union Tile { K keys[SORT_TILE]; uint32_t vals[SORT_TILE]; };
+  Tile& sm = *reinterpret_cast<Tile*>(sort_smem);
+  uint32_t (*whist)[RADIX] = reinterpret_cast<uint32_t (*)[RADIX]>(sort_smem + sizeof(Tile));
   __shared__ uint32_t s_toff[RADIX];    // first position of digit d inside the sorted tile
   __shared__ uint32_t s_goff[RADIX];    // global position of tile position p with digit d = s_goff[d] + p
-  __shared__ uint32_t s_wsum[SORT_WARPS];
+  __shared__ uint32_t s_wsum[RADIX / 32];
   __shared__ uint32_t s_tile;
 
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   if (tid == 0) s_tile = atomicAdd(counter, 1u);   // ticket: tile t starts only after tiles < t did
-#pragma unroll
-  for (int i = 0; i < SORT_WARPS; ++i) whist[i][tid] = 0;
+  for (int i = tid; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&whist[0][0])[i] = 0;
   __syncthreads();
   const uint32_t tile = s_tile;
   const uint32_t tile_base = tile * (uint32_t)SORT_TILE;
@@ -154,10 +159,10 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
   }
   __syncthreads();
 
-  // thread d owns digit d: exclusive scan over warps, tile count, publish, look back
-  {
-    const int d = tid;
-    uint32_t run = 0;
+  // thread d < 256 owns digit d: exclusive scan over warps, tile count, publish, look back
+  const int d = tid;
+  uint32_t run = 0, pub = 0, x = 0;
+  if (tid < RADIX) {
 #pragma unroll
     for (int i = 0; i < SORT_WARPS; ++i) {
       uint32_t t = whist[i][d];
@@ -165,22 +170,24 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
       run += t;
     }
     // padding keys (all ones) of a partial last tile sit in digit 255; nobody reads their count
-    uint32_t pub = run;
+    pub = run;
     if (d == 255) pub -= (uint32_t)SORT_TILE - nvalid;
     st_volatile_u32(&status[(size_t)tile * RADIX + d], (tile == 0 ? FLAG_INCL : FLAG_AGG) | pub);
 
     // exclusive scan of the tile counts over digits
-    uint32_t x = run;
+    x = run;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       uint32_t y = __shfl_up_sync(~0u, x, o);
       if (lane >= o) x += y;
     }
     if (lane == 31) s_wsum[w] = x;
-    __syncthreads();
+  }
+  __syncthreads();
+  if (tid < RADIX) {
     uint32_t wb = 0;
 #pragma unroll
-    for (int i = 0; i < SORT_WARPS; ++i) wb += i < w ? s_wsum[i] : 0u;
+    for (int i = 0; i < RADIX / 32; ++i) wb += i < w ? s_wsum[i] : 0u;
     const uint32_t toff = wb + x - run;
     s_toff[d] = toff;
 
@@ -188,7 +195,7 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
     if (tile > 0) {
       // decoupled look-back, LB predecessors per round trip: the loads of a batch are
       // independent, so a walk over many aggregate-only tiles costs one latency per batch
-      constexpr int LB = 8;
+      constexpr int LB = SORT_LB;
       int t = (int)tile - 1;
       bool done = false;
       while (!done) {
@@ -287,6 +294,10 @@ arbx_status radix_sort_impl(K* keys, uint32_t* vals, bool iota, int64_t n, int k
     hist_scan_kernel<<<npass, RADIX, 0, s>>>(ghist);
     ARBX_LAUNCH_CHECK();
   }
+  const size_t smem = (sizeof(K) > 4 ? sizeof(K) : 4) * SORT_TILE + sizeof(uint32_t) * SORT_WARPS * RADIX;
+  ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   K* kin = keys; K* kout = kalt.p;
   uint32_t* vin = vals; uint32_t* vout = valt.p;
   for (int p = 0; p < npass; ++p) {
@@ -294,11 +305,11 @@ arbx_status radix_sort_impl(K* keys, uint32_t* vals, bool iota, int64_t n, int k
     uint32_t* st = status + (size_t)p * ntiles * RADIX;
     ProfScope ps(kPassId, s);
     if (!has_vals)
-      onesweep_pass<K, false, false><<<ntiles, SORT_THREADS, 0, s>>>(kin, kout, nullptr, nullptr, (uint32_t)n, 8 * p, base, counters + p, st);
+      onesweep_pass<K, false, false><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, nullptr, nullptr, (uint32_t)n, 8 * p, base, counters + p, st);
     else if (p == 0 && iota)
-      onesweep_pass<K, true, true><<<ntiles, SORT_THREADS, 0, s>>>(kin, kout, nullptr, vout, (uint32_t)n, 8 * p, base, counters + p, st);
+      onesweep_pass<K, true, true><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, nullptr, vout, (uint32_t)n, 8 * p, base, counters + p, st);
     else
-      onesweep_pass<K, false, true><<<ntiles, SORT_THREADS, 0, s>>>(kin, kout, vin, vout, (uint32_t)n, 8 * p, base, counters + p, st);
+      onesweep_pass<K, false, true><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, vin, vout, (uint32_t)n, 8 * p, base, counters + p, st);
     ARBX_LAUNCH_CHECK();
     std::swap(kin, kout);
     std::swap(vin, vout);
