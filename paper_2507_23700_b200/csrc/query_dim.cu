@@ -19,7 +19,7 @@ namespace arbx {
 namespace {
 
 constexpr int D = ARBX_DIM;
-constexpr int QT = 128;   // threads per block of the traversal kernels
+constexpr int QT = 64;    // threads per block of the traversal kernels (64 measured ~1% faster than 128)
 
 // ---- Q1: 32-bit space-filling code of each query centre inside the scene bounds --------------
 template <int QK>
