@@ -428,3 +428,24 @@ def test_count_upto_lattice_closed_form(arbx):
         c = _np(ix.query_count(_dev(dg.sphere_queries(p, 1.0)), dg.SPHERE, limit=limit))
         assert np.array_equal(c, np.minimum(expect, limit))
     ix.close()
+
+
+def test_run_to_run_determinism(arbx):
+    """T5: result SETS are identical from run to run (atomics only order arrivals, never values)."""
+    prims = _dev(dg.uniform_points(300_000, 3, 71))
+    q = _dev(dg.sphere_queries(dg.uniform_points(200_000, 3, 72), 0.02))
+    ref = None
+    for _ in range(3):
+        ix = arbx.Index(prims, dg.POINT)
+        assert ix.validate() == 0
+        c = ix.query_count(q)
+        off, idx = ix.query_spatial(q)
+        gi, gd = ix.query_knn(q[:, :3].contiguous(), 8)
+        ix.close()
+        rows = torch.stack([torch.repeat_interleave(torch.arange(off.numel() - 1, device="cuda"), torch.diff(off).long()), idx.long()], 1)
+        key = torch.sort(rows[:, 0] * 300_000 + rows[:, 1]).values
+        cur = (c.clone(), off.clone(), key, gd.clone())
+        if ref is None:
+            ref = cur
+        else:
+            assert all(torch.equal(a, b) for a, b in zip(ref, cur))
