@@ -268,6 +268,18 @@ __device__ __forceinline__ bool joint_hits_prim(const Joint<QK>& J, const float*
   }
 }
 
+template <int QK>
+__device__ __forceinline__ bool joint_hits_box(const Joint<QK>& J, const float* lo, const float* hi) {
+  if constexpr (QK == KIND_SPHERE) {
+    return dist2_bb<D>(lo, hi, J.lo, J.hi) <= J.r2;
+  } else {
+    bool ok = true;
+#pragma unroll
+    for (int a = 0; a < D; ++a) ok = ok && lo[a] <= J.hi[a] && J.lo[a] <= hi[a];
+    return ok;
+  }
+}
+
 struct NodeX { float v[4 * D]; int32_t c0, c1, l, r; };
 
 __device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, int32_t ref, NodeX& nd) {
@@ -297,7 +309,8 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
                                                      int* __restrict__ overflow, int mode, float alpha) {
   constexpr bool FILL = MODE != 0;     // hits are written somewhere
   constexpr int QW = prim_width(QK, D);
-  __shared__ int32_t s_stack[QT / 32][STACK_DEPTH];
+  constexpr int PQ_CAP = 320;   // packet work list (node ids) per warp
+  __shared__ int32_t s_stack[QT / 32][PQ_CAP];
   int32_t* stack = s_stack[threadIdx.x >> 5];
   const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
   const bool valid = t < nq;
@@ -391,30 +404,53 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
     if constexpr (MODE == 0) { if (cnt >= limit) alive = false; }   // capped count: seen enough
   };
 
+  // Node work is spread over the lanes: the warp keeps a work list of node ids in shared
+  // memory, pops up to 32 of them, and lane i tests the two child boxes of node i against the
+  // JOINT region.  Hit leaf-range children are scanned on the spot (warp-uniform loop over the
+  // ballot), hit internal children are compacted back onto the list.  When the list runs
+  // close to its capacity the warp pops one node at a time, which bounds growth by the tree depth.
   if (__any_sync(~0u, alive)) {
-    int32_t ref = __ldg(root);
-    if (ref < 0) {
+    const int32_t rootref = __ldg(root);
+    if (rootref < 0) {
       leaf_range(0, n);
     } else {
-      int sp = 0;
-      for (;;) {
+      const uint32_t lt = (1u << lane) - 1u;
+      int nlist = 1;
+      stack[0] = rootref;
+      __syncwarp();
+      while (nlist > 0) {
+        const int take = nlist > PQ_CAP - STACK_DEPTH - 64 ? 1 : min(32, nlist);
+        nlist -= take;
+        const int32_t my = lane < take ? stack[nlist + lane] : -1;
+        __syncwarp();
         NodeX nd;
-        load_node_x(nodes, ref, nd);
-        const bool a0 = __any_sync(~0u, alive && hits_box<QK>(q, nd.v, nd.v + D));
-        const bool a1 = __any_sync(~0u, alive && hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D));
-        if (a0 && nd.c0 < 0) leaf_range(nd.l, ref - nd.l + 1);
-        if (a1 && nd.c1 < 0) leaf_range(ref + 1, nd.r - ref);
-        if constexpr (MODE == 0) { if (cap > 0 && !__any_sync(~0u, alive)) break; }
-        const bool in0 = a0 && nd.c0 >= 0, in1 = a1 && nd.c1 >= 0;
-        if (in0) {
-          ref = nd.c0;
-          if (in1) stack[sp++] = nd.c1;
-        } else if (in1) {
-          ref = nd.c1;
-        } else {
-          if (sp == 0) break;
-          ref = stack[--sp];
+        bool in0 = false, in1 = false, lf0 = false, lf1 = false;
+        if (my >= 0) {
+          load_node_x(nodes, my, nd);
+          const bool h0 = joint_hits_box<QK>(J, nd.v, nd.v + D);
+          const bool h1 = joint_hits_box<QK>(J, nd.v + 2 * D, nd.v + 3 * D);
+          in0 = h0 && nd.c0 >= 0; lf0 = h0 && nd.c0 < 0;
+          in1 = h1 && nd.c1 >= 0; lf1 = h1 && nd.c1 < 0;
         }
+        uint32_t m0 = __ballot_sync(~0u, lf0), m1 = __ballot_sync(~0u, lf1);
+        while (m0) {
+          const int b = __ffs(m0) - 1;
+          m0 &= m0 - 1;
+          const int l = __shfl_sync(~0u, nd.l, b), p = __shfl_sync(~0u, my, b);
+          leaf_range(l, p - l + 1);
+        }
+        while (m1) {
+          const int b = __ffs(m1) - 1;
+          m1 &= m1 - 1;
+          const int r = __shfl_sync(~0u, nd.r, b), p = __shfl_sync(~0u, my, b);
+          leaf_range(p + 1, r - p);
+        }
+        if constexpr (MODE == 0) { if (cap > 0 && !__any_sync(~0u, alive)) break; }
+        const uint32_t b0 = __ballot_sync(~0u, in0), b1 = __ballot_sync(~0u, in1);
+        if (in0) stack[nlist + __popc(b0 & lt)] = nd.c0;
+        if (in1) stack[nlist + __popc(b0) + __popc(b1 & lt)] = nd.c1;
+        nlist += __popc(b0) + __popc(b1);
+        __syncwarp();
       }
     }
   }
@@ -733,7 +769,9 @@ arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s
   const float4* leaves = reinterpret_cast<const float4*>(ix->leaves);
   ProfScope ps(a.pass == 1 ? K_SPATIAL_FILL : K_SPATIAL_COUNT, s);
   const int mode = traversal_mode();
-  float alpha = 0.75f;
+  // packet threshold (spread of the warp's query centres <= alpha * query extent), measured:
+  // 1.5 (spheres) / 2.5 (boxes) up to 3-D, 0.75 above (the joint region gets loose quickly)
+  float alpha = D <= 3 ? (QK == KIND_BOX ? 2.5f : 1.5f) : 0.75f;
   if (const char* v = getenv("ARBX_PACKET_ALPHA")) alpha = (float)atof(v);
   const int n = (int)ix->n;
   if (a.pass == 1)
