@@ -161,8 +161,9 @@ __device__ __forceinline__ int block_running_max(int v, int* s_w) {
 template <int D, int PK>
 __global__ void __launch_bounds__(HierCfg<D>::HB)
 hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict__ leaves,
-                 float* __restrict__ nodes, int* __restrict__ flags, int n, int leaf_max,
-                 int32_t* __restrict__ root) {
+                 float* __restrict__ nodes, int n, int leaf_max, int32_t* __restrict__ root,
+                 int* __restrict__ open_count, int* __restrict__ open_lrf, float* __restrict__ open_box,
+                 int open_cap) {
   constexpr int HB = HierCfg<D>::HB;
   constexpr int W = prim_width(PK, D);
   constexpr int LW = leaf_width(PK, D);
@@ -188,23 +189,52 @@ hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict
     s_suf[HB - tid] = (uint8_t)sm;
   }
   __syncthreads();
-  if (i >= n) return;
 
+  // Leaf ranges first, from the level bytes alone (no atomics, no boxes).  Split j is the top
+  // of a subtree [l_j, r_j] bounded by the nearest higher level on each side; it is a leaf-
+  // range BOUNDARY iff that subtree holds more than leaf_max primitives.  Every thread
+  // classifies one split with two short scans; then the thread of each range's first leaf
+  // scans the range for its box and starts the climb there.  The merges below leaf-range
+  // level (the bulk of all merges) never happen.
+  auto lvl = [&](int j) -> int {   // level of split j, -1 <= j <= n-1
+    const int t = j - (c0 - 1);
+    return (t >= 0 && t <= HB) ? (int)s_lvl[t] : split_level(codes, j, n);
+  };
+  auto is_boundary = [&](int j) -> bool {
+    const int L = lvl(j);
+    if (L == 255) return true;
+    int da = 1, db = 1;          // steps to the nearest higher level on the left / right
+    while (da <= leaf_max && lvl(j - da) < L) ++da;
+    while (da + db <= leaf_max && lvl(j + db) < L) ++db;
+    return da + db > leaf_max;   // subtree size = da + db
+  };
+  __shared__ uint8_t s_bnd[HB + 1];
+  s_bnd[tid] = is_boundary(c0 - 1 + tid) ? 1 : 0;
+  if (tid == 0) s_bnd[HB] = is_boundary(c0 - 1 + HB) ? 1 : 0;
+  __syncthreads();
+  if (i >= n || !s_bnd[tid]) return;     // not the first leaf of a range
   int l = i, r = i;
-  int32_t ref = ~i;
+  for (;; ++r) {                         // the range ends at the next boundary split
+    const int t = r - c0 + 1;
+    if (t <= HB ? s_bnd[t] != 0 : is_boundary(r)) break;
+  }
+  int32_t ref = ~l;
   float lo[D], hi[D];
-  {
-    float v[W];
-    const float* lf = leaves + (int64_t)i * LW;
+#pragma unroll
+  for (int a = 0; a < D; ++a) { lo[a] = INFINITY; hi[a] = -INFINITY; }
+  for (int j = l; j <= r; ++j) {
+    float v[W], bl[D], bh[D];
+    const float* lf = leaves + (int64_t)j * LW;
 #pragma unroll
     for (int e = 0; e < W; ++e) v[e] = lf[e];
-    box_of<D, PK>(v, lo, hi);
+    box_of<D, PK>(v, bl, bh);
+#pragma unroll
+    for (int a = 0; a < D; ++a) { lo[a] = fminf(lo[a], bl[a]); hi[a] = fmaxf(hi[a], bh[a]); }
   }
-  uint32_t* leaf_idx = reinterpret_cast<uint32_t*>(leaves);
+  reinterpret_cast<uint32_t*>(leaves)[(int64_t)r * LW + W] |= LEAF_END;   // last record of the range
   for (;;) {
     if (l == 0 && r == n - 1) {   // root
       *root = ref;
-      if (ref < 0) leaf_idx[(int64_t)r * LW + W] |= LEAF_END;
       return;
     }
     // the parent splits either right after r (we are its left child) or right before l
@@ -227,44 +257,80 @@ hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict
       }
       __stcg(reinterpret_cast<int*>(node) + 4 * D + slot, ref);
     };
-    int other;
-    if (local) {
-      // the sibling reads our box from shared memory, so the global stores stay outside the
-      // fence -> atomic window (a fence would otherwise wait for them)
-      float* mine = s_box[slot][p - c0];
+    if (!local) {
+      // The parent reaches outside this chunk: park the subtree for hierarchy_top_kernel, so
+      // that this block is not kept alive by a chain of global round trips.
+      const int e = atomicAdd(open_count, 1);
+      if (e < open_cap) {
+        open_lrf[3 * e] = l; open_lrf[3 * e + 1] = r; open_lrf[3 * e + 2] = ref;
 #pragma unroll
-      for (int a = 0; a < D; ++a) { mine[a] = lo[a]; mine[D + a] = hi[a]; }
-      __threadfence_block();
-      other = atomicExch(&s_flag[p - c0], left_child ? l : r);
-      store_half();
-      if (other == -1) return;   // first to arrive: the sibling's thread carries on
-      __threadfence_block();
-      const volatile float* theirs = s_box[sib][p - c0];
-#pragma unroll
-      for (int a = 0; a < D; ++a) { lo[a] = fminf(lo[a], theirs[a]); hi[a] = fmaxf(hi[a], theirs[D + a]); }
-    } else {
-      store_half();
-      __threadfence();
-      other = atomicExch(flags + p, left_child ? l : r);
-      if (other == -1) return;
-      __threadfence();
-#pragma unroll
-      for (int a = 0; a < D; ++a) {
-        lo[a] = fminf(lo[a], __ldcg(node + sib * 2 * D + a));
-        hi[a] = fmaxf(hi[a], __ldcg(node + sib * 2 * D + D + a));
+        for (int a = 0; a < D; ++a) { open_box[(int64_t)e * 2 * D + a] = lo[a]; open_box[(int64_t)e * 2 * D + D + a] = hi[a]; }
       }
+      return;
     }
+    // the sibling reads our box from shared memory, so the global stores stay outside the
+    // fence -> atomic window (a fence would otherwise wait for them)
+    float* mine = s_box[slot][p - c0];
+#pragma unroll
+    for (int a = 0; a < D; ++a) { mine[a] = lo[a]; mine[D + a] = hi[a]; }
+    __threadfence_block();
+    const int other = atomicExch(&s_flag[p - c0], left_child ? l : r);
+    store_half();
+    if (other == -1) return;   // first to arrive: the sibling's thread carries on
+    __threadfence_block();
+    const volatile float* theirs = s_box[sib][p - c0];
+#pragma unroll
+    for (int a = 0; a < D; ++a) { lo[a] = fminf(lo[a], theirs[a]); hi[a] = fmaxf(hi[a], theirs[D + a]); }
     // second to arrive: `other` is the far end of the sibling's range
     if (left_child) r = other; else l = other;
     __stcg(reinterpret_cast<int*>(node) + 4 * D + 2, l);
     __stcg(reinterpret_cast<int*>(node) + 4 * D + 3, r);
-    if (r - l + 1 <= leaf_max) {
-      ref = ~l;                  // collapsed subtree: a leaf range, node p stays unused
-    } else {
-      ref = p;
-      if (p - l + 1 <= leaf_max) leaf_idx[(int64_t)p * LW + W] |= LEAF_END;
-      if (r - p <= leaf_max) leaf_idx[(int64_t)r * LW + W] |= LEAF_END;
+    ref = p;   // leaf ranges are maximal, so every merge makes a real node
+  }
+}
+
+// Top of the tree: one thread per parked subtree, every merge through global memory (node
+// record + atomicExch flag + __threadfence), the classic bottom-up scheme.  Only O(log chunk)
+// subtrees per chunk get here.
+template <int D>
+__global__ void __launch_bounds__(256)
+hierarchy_top_kernel(const unsigned long long* __restrict__ codes, float* __restrict__ nodes,
+                     int* __restrict__ flags, int n, int32_t* __restrict__ root,
+                     const int* __restrict__ open_count, const int* __restrict__ open_lrf,
+                     const float* __restrict__ open_box, int open_cap) {
+  constexpr int NW = node_width(D);
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= min(*open_count, open_cap)) return;
+  int l = open_lrf[3 * e], r = open_lrf[3 * e + 1];
+  int32_t ref = open_lrf[3 * e + 2];
+  float lo[D], hi[D];
+#pragma unroll
+  for (int a = 0; a < D; ++a) { lo[a] = open_box[(int64_t)e * 2 * D + a]; hi[a] = open_box[(int64_t)e * 2 * D + D + a]; }
+  for (;;) {
+    if (l == 0 && r == n - 1) { *root = ref; return; }
+    const bool left_child = split_level(codes, r, n) < split_level(codes, l - 1, n);
+    const int p = left_child ? r : l - 1;
+    float* node = nodes + (int64_t)p * NW;
+    const int slot = left_child ? 0 : 1, sib = 1 - slot;
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+      __stcg(node + slot * 2 * D + a, lo[a]);
+      __stcg(node + slot * 2 * D + D + a, hi[a]);
     }
+    __stcg(reinterpret_cast<int*>(node) + 4 * D + slot, ref);
+    __threadfence();
+    const int other = atomicExch(flags + p, left_child ? l : r);
+    if (other == -1) return;     // first to arrive: the sibling's thread carries on
+    __threadfence();
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+      lo[a] = fminf(lo[a], __ldcg(node + sib * 2 * D + a));
+      hi[a] = fmaxf(hi[a], __ldcg(node + sib * 2 * D + D + a));
+    }
+    if (left_child) r = other; else l = other;
+    __stcg(reinterpret_cast<int*>(node) + 4 * D + 2, l);
+    __stcg(reinterpret_cast<int*>(node) + 4 * D + 3, r);
+    ref = p;
   }
 }
 
@@ -307,10 +373,22 @@ arbx_status build_typed(const float* prims, int64_t n, cudaStream_t s, Index* ix
   ARBX_TRY(scratch_alloc((void**)&ix->nodes, nn * NW * sizeof(float), s));
   ARBX_TRY(flags.alloc(nn, s));
   ProfScope ps(K_HIERARCHY, s);
-  ARBX_CUDA(cudaMemsetAsync(flags.p, 0xff, nn * sizeof(int), s));
   constexpr int HB = HierCfg<D>::HB;
-  hierarchy_kernel<D, PK><<<(unsigned)((n + HB - 1) / HB), HB, 0, s>>>(ix->codes, ix->leaves, ix->nodes, flags.p,
-                                                                      (int)n, ix->leaf_max, ix->root);
+  const unsigned nchunks = (unsigned)((n + HB - 1) / HB);
+  // at most one parked subtree per distinct prefix / suffix maximum of the level bytes of a chunk
+  const int64_t open_cap = std::min<int64_t>(n, (int64_t)nchunks * 200);
+  Scratch<int> open_lrf, open_count;
+  Scratch<float> open_box;
+  ARBX_TRY(open_count.alloc(1, s));
+  ARBX_TRY(open_lrf.alloc((size_t)open_cap * 3, s));
+  ARBX_TRY(open_box.alloc((size_t)open_cap * 2 * D, s));
+  ARBX_CUDA(cudaMemsetAsync(open_count.p, 0, sizeof(int), s));
+  ARBX_CUDA(cudaMemsetAsync(flags.p, 0xff, nn * sizeof(int), s));
+  hierarchy_kernel<D, PK><<<nchunks, HB, 0, s>>>(ix->codes, ix->leaves, ix->nodes, (int)n, ix->leaf_max, ix->root,
+                                                 open_count.p, open_lrf.p, open_box.p, (int)open_cap);
+  ARBX_LAUNCH_CHECK();
+  hierarchy_top_kernel<D><<<(unsigned)((open_cap + 255) / 256), 256, 0, s>>>(ix->codes, ix->nodes, flags.p, (int)n, ix->root,
+                                                                           open_count.p, open_lrf.p, open_box.p, (int)open_cap);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }

@@ -86,9 +86,12 @@ __global__ void v_nodes_kernel(const float* leaves, const float* nodes, int n, i
   if (p >= n - 1) return;
   const float* nd = nodes + (int64_t)p * NW;
   const int* ni = reinterpret_cast<const int*>(nd) + 4 * D;
+  // a split inside a leaf range has no node (its slot is never written): leaf p does not carry
+  // the end-of-range mark
+  if (!(__float_as_uint(leaves[(int64_t)p * leaf_width(PK, D) + prim_width(PK, D)]) & LEAF_END)) return;
   const int l = ni[2], r = ni[3];
   if (l < 0 || r >= n || l > p || r <= p) { fail(viol); return; }
-  if (r - l + 1 <= leaf_max) return;   // collapsed into a leaf range: slot unused
+  if (r - l + 1 <= leaf_max) { fail(viol); return; }   // leaf ranges are maximal
   real[p] = 1;
   check_child<D, PK>(leaves, nodes, ni[0], l, p, n, leaf_max, nd, nd + D, refcnt, cover, viol);
   check_child<D, PK>(leaves, nodes, ni[1], p + 1, r, n, leaf_max, nd + 2 * D, nd + 3 * D, refcnt, cover, viol);
