@@ -359,6 +359,21 @@ def main():
     calls = {c: v / args.steps for c, v in calls.items()}
     marks.clear()
 
+    # ---- outside the step: the capped count (NEXT-1, arbx_query_count_upto), device-timed ---------------
+    extras = {}
+    with torch.cuda.stream(stream):
+        hx = arbx.arbx_build(d_prims, D, pk, stream)
+        for limit in (1, 8):
+            for rep in range(3):
+                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                arbx.arbx_query_count_upto(hx, d_queries, nq, qk, limit, counts, stream)
+                b.record(stream)
+            torch.cuda.synchronize()
+            extras[f"count_upto_{limit}_qps"] = round(nq / a.elapsed_time(b) * 1e3, 1)
+        arbx.arbx_destroy(hx, stream)
+    torch.cuda.synchronize()
+
     # ---- e2e leg: pinned host inputs in, every result back to pinned host memory ---------------------
     e2e = None
     if not args.no_e2e:
@@ -430,7 +445,7 @@ def main():
             radius_csr_qps=round(nq / calls["spatial"] * 1e3, 1), radius_csr_ms=round(calls["spatial"], 4),
             count_only_qps=round(nq / calls["count"] * 1e3, 1), count_only_ms=round(calls["count"], 4),
             knn_qps=round(nq / calls["knn"] * 1e3, 1) if k else None, knn_ms=round(calls["knn"], 4) if k else None,
-            pairs=capacity, kernels=kern)
+            pairs=capacity, extras_outside_step=extras, kernels=kern)
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             import oracle
