@@ -116,6 +116,14 @@ ARBX_API arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int
                                int32_t* offsets, int32_t* indices, int64_t indices_capacity,
                                int64_t* total_host, arbx_stream stream);
 
+/* Capped storage search: as arbx_query_spatial, but every query keeps at most `limit`
+ * (>= 1) of its matches and stops its traversal there (PAPER.md:L174 early_exit from a
+ * callback that stores).  offsets[q+1]-offsets[q] = min(matches of q, limit); WHICH matches
+ * are kept is unspecified (traversal order).  Same capacity protocol and errors.            */
+ARBX_API arbx_status arbx_query_spatial_upto(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                                    int32_t limit, int32_t* offsets, int32_t* indices,
+                                    int64_t indices_capacity, int64_t* total_host, arbx_stream stream);
+
 /* k nearest primitives to each query point ("a pair of a query point and a
  * number of neighbors"; L79 distance to the stored geometry: point ||x-y||, box point-box
  * distance (0 inside), sphere max(0,||y-c||-R)).  qpoints: DEVICE nq*dim.  One k per call,

@@ -123,3 +123,18 @@ def compare_counts_upto(orc, counts, limit: int, what: str = "") -> None:
     lo, hi = np.minimum(allc - bandc, limit), np.minimum(allc, limit)
     bad = (counts < lo) | (counts > hi)
     assert not bad.any(), f"{what}: {int(bad.sum())} capped counts outside [min(sure,L), min(sure+band,L)], first q={int(np.argmax(bad))}"
+
+
+def compare_spatial_upto(n: int, orc, got, limit: int, what: str = "") -> None:
+    """Capped storage query: every reported pair is a (sure or band) pair of the full oracle
+    result, rows are duplicate-free, and row sizes obey the capped-count rule."""
+    o_off, o_idx, _ = orc
+    g_off, g_idx = got
+    nq = len(o_off) - 1
+    check_csr_format(g_off, g_idx, n, nq)
+    ko = _keys(o_off, o_idx, n)
+    kg = np.sort(_keys(g_off, g_idx, n))
+    assert np.all(np.diff(kg) > 0), f"{what}: duplicate index inside a row"
+    extra = ~np.isin(kg, ko, assume_unique=True)
+    assert not extra.any(), f"{what}: {int(extra.sum())} reported pairs are not matches"
+    compare_counts_upto(orc, np.diff(np.asarray(g_off, dtype=np.int64)), limit, what)

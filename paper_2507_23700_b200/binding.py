@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libarbx.so")
 
 EXPORTS = (
     "arbx_build", "arbx_destroy", "arbx_size", "arbx_bounds", "arbx_query_count",
-    "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
+    "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_spatial_upto", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
     "arbx_launch_count", "arbx_profile_enable", "arbx_profile_num_kernels",
     "arbx_profile_kernel_name", "arbx_profile_read", "arbx_status_string", "arbx_last_error",
 )
@@ -56,6 +56,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_query_count.argtypes = [vp, vp, i64, i32, vp, vp]
         L.arbx_query_count_upto.argtypes = [vp, vp, i64, i32, i32, vp, vp]
         L.arbx_query_spatial.argtypes = [vp, vp, i64, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.arbx_query_spatial_upto.argtypes = [vp, vp, i64, i32, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.arbx_query_knn.argtypes = [vp, vp, i64, i32, vp, vp, vp]
         L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
         L.arbx_debug_validate.argtypes = [vp, ctypes.POINTER(i64), vp]
@@ -70,7 +71,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_status_string.restype = ctypes.c_char_p
         L.arbx_status_string.argtypes = [i32]
         L.arbx_last_error.restype = ctypes.c_char_p
-        for name in EXPORTS[:10]:
+        for name in EXPORTS[:11]:
             getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -150,6 +151,18 @@ def arbx_query_spatial(handle: int, queries: torch.Tensor, nq: int, qkind: int, 
                                   ctypes.byref(total), _stream(stream))
     if st != OK and (raise_on_capacity or st != ERR_CAPACITY):
         raise ArbxError(st, "arbx_query_spatial")
+    return st, total.value
+
+
+def arbx_query_spatial_upto(handle: int, queries: torch.Tensor, nq: int, qkind: int, limit: int,
+                            offsets: torch.Tensor, indices, capacity: int, stream=None):
+    """Returns (status, total); ERR_CAPACITY is returned, not raised."""
+    total = ctypes.c_int64()
+    st = lib().arbx_query_spatial_upto(handle, _ptr(queries), nq, qkind, limit, offsets.data_ptr(),
+                                       0 if indices is None else indices.data_ptr(), capacity,
+                                       ctypes.byref(total), _stream(stream))
+    if st not in (OK, ERR_CAPACITY):
+        raise ArbxError(st, "arbx_query_spatial_upto")
     return st, total.value
 
 
@@ -257,6 +270,15 @@ class Index:
         indices = torch.empty(total, dtype=torch.int32, device=self.device)
         arbx_query_spatial(self.handle, queries, nq, qkind, offsets, indices, total, stream)
         return offsets, indices
+
+    def query_spatial_upto(self, queries: torch.Tensor, limit: int, qkind: int = SPHERE, stream=None):
+        """CSR result with at most `limit` matches per query (early exit)."""
+        nq = self._nq(queries, qkind)
+        offsets = torch.empty(nq + 1, dtype=torch.int32, device=self.device)
+        indices = torch.empty(max(nq * limit, 1), dtype=torch.int32, device=self.device)
+        _, total = arbx_query_spatial_upto(self.handle, queries, nq, qkind, limit, offsets, indices,
+                                           indices.numel(), stream)
+        return offsets, indices[:total]
 
     def query_knn(self, qpoints: torch.Tensor, k: int, want_distances: bool = True, stream=None):
         nq = self._nq(qpoints, POINT)

@@ -218,9 +218,26 @@ static arbx_status count_impl(arbx_handle h, const float* queries, int64_t nq, a
   return dim_table(ix->dim)->spatial(ix, a, s);
 }
 
+static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind, int32_t limit,
+                                int32_t* offsets, int32_t* indices, int64_t indices_capacity,
+                                int64_t* total_host, arbx_stream stream);
+
 arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
                                int32_t* offsets, int32_t* indices, int64_t indices_capacity,
                                int64_t* total_host, arbx_stream stream) {
+  return spatial_impl(h, queries, nq, qkind, 0, offsets, indices, indices_capacity, total_host, stream);
+}
+
+arbx_status arbx_query_spatial_upto(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                                    int32_t limit, int32_t* offsets, int32_t* indices,
+                                    int64_t indices_capacity, int64_t* total_host, arbx_stream stream) {
+  if (limit < 1) { set_error("arbx_query_spatial_upto: limit must be >= 1"); return ARBX_ERR_INVALID_ARG; }
+  return spatial_impl(h, queries, nq, qkind, limit, offsets, indices, indices_capacity, total_host, stream);
+}
+
+static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind, int32_t limit,
+                                int32_t* offsets, int32_t* indices, int64_t indices_capacity,
+                                int64_t* total_host, arbx_stream stream) {
   if (!h || nq < 0 || bad_kind((int)qkind) || !offsets || (nq > 0 && !queries) || indices_capacity < 0) {
     set_error("arbx_query_spatial: invalid argument");
     return ARBX_ERR_INVALID_ARG;
@@ -245,13 +262,15 @@ arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, 
   // `cap` matches of every query in a scratch row; after the scan the rows are copied into
   // their CSR slices and only queries with more than cap matches are traversed again.
   int cap = 0;
-  if (indices) {
+  if (indices && limit == 0) {
     const long long budget = (long long)env_int("ARBX_STORE_BUDGET_MB", 4096) << 20;
     for (int c = 64; c >= 16 && cap == 0; c >>= 1)
       if ((long long)nq * c * 4 <= budget) cap = c;
   }
   SpatialArgs a{queries, nq, (int)qkind, order.p, counts.p, nullptr, nullptr, nullptr, cap,
                 reinterpret_cast<int*>(total_dev.p + 1), cap ? 2 : 0};
+  // capped storage query: capped count (early exit) -> scan -> fill that stops at each count
+  if (limit > 0) a.cap = limit;
   if (cap) {
     ARBX_TRY(rows.alloc((size_t)nq * cap, s));
     a.rows = rows.p;
@@ -277,6 +296,7 @@ arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, 
   a.offsets = offsets;
   a.indices = indices;
   a.pass = 1;
+  if (limit > 0) { a.cap = 0; a.stop_fill = 1; }
   if (cap) {
     ARBX_TRY(compact_rows(rows.p, cap, counts.p, offsets, indices, nq, s));
     if (noverflow == 0) return ARBX_OK;

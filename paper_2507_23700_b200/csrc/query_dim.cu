@@ -146,7 +146,7 @@ __device__ __forceinline__ bool hits_prim(const Query<QK>& q, const float* p) {
 template <int PK, int QK, bool FILL>
 __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes, const float4* __restrict__ leaves,
                                                const int32_t* __restrict__ root, const Query<QK>& q,
-                                               int32_t* __restrict__ out, int limit) {
+                                               int32_t* __restrict__ out, int limit, int stop) {
   int cnt = 0;
   int32_t stack[STACK_DEPTH];
   int sp = 0;
@@ -175,7 +175,7 @@ __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes,
       if (hits_prim<QK, PK>(q, lf.v)) {
         if constexpr (FILL) { if (cnt < limit) out[cnt] = (int32_t)(lf.idx & ~LEAF_END); }
         ++cnt;
-        if constexpr (!FILL) { if (cnt >= limit) return cnt; }   // capped count: early exit
+        if (cnt >= stop) return cnt;   // capped query: early exit
       }
       if (lf.idx & LEAF_END) break;
     }
@@ -306,7 +306,8 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
                                                      int32_t* __restrict__ counts,
                                                      const int32_t* __restrict__ offsets,
                                                      int32_t* __restrict__ indices, int cap,
-                                                     int* __restrict__ overflow, int mode, float alpha) {
+                                                     int* __restrict__ overflow, int stop_fill, int mode,
+                                                     float alpha) {
   constexpr bool FILL = MODE != 0;     // hits are written somewhere
   constexpr int QW = prim_width(QK, D);
   constexpr int PQ_CAP = 320;   // packet work list (node ids) per warp
@@ -331,15 +332,23 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   }
   int64_t base64 = 0;   // where this query's hits go in `indices` (MODE 1: CSR slice, MODE 2: row q*cap)
   int limit = INT32_MAX;
+  bool capped = false;   // this lane stops after `limit` hits (capped count / capped fill)
   if constexpr (MODE == 1) {
     base64 = valid ? offsets[qi] : 0;
+    if (stop_fill) {     // capped storage query: write exactly the counted number of hits
+      limit = valid ? counts[qi] : 0;
+      alive = alive && limit > 0;
+      capped = true;
+      if (!__any_sync(~0u, alive)) return;
+    }
   }
   if constexpr (MODE == 2) { base64 = qi * cap; limit = cap; }
-  if constexpr (MODE == 0) { if (cap > 0) limit = cap; }   // capped count (arbx_query_count_upto)
+  if constexpr (MODE == 0) { if (cap > 0) { limit = cap; capped = true; } }   // arbx_query_count_upto
   // mode 0: per-warp choice; 1: always one query per lane; 2: always packet
   if (mode == 1 || (mode == 0 && !warp_coherent<QK>(q, valid, alpha))) {
     int c = 0;
-    if (alive) c = thread_traverse<PK, QK, FILL>(nodes, leaves, root, q, FILL ? indices + base64 : nullptr, limit);
+    if (alive) c = thread_traverse<PK, QK, FILL>(nodes, leaves, root, q, FILL ? indices + base64 : nullptr, limit,
+                                                  capped ? limit : INT32_MAX);
     if constexpr (MODE != 1) {
       if (valid) counts[qi] = c;
       if constexpr (MODE == 2) { if (c > cap) atomicAdd(overflow, 1); }
@@ -393,7 +402,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
           const uint32_t full = __ballot_sync(~0u, pend == FS);
           if (full) flush(full);
           if (hit) {
-            if (MODE == 1 || cnt < limit) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
+            if (cnt < limit) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
             ++cnt;
           }
         } else {
@@ -401,7 +410,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
         }
       }
     }
-    if constexpr (MODE == 0) { if (cnt >= limit) alive = false; }   // capped count: seen enough
+    if (capped && cnt >= limit) alive = false;   // capped query: this lane has seen enough
   };
 
   // Node work is spread over the lanes: the warp keeps a work list of node ids in shared
@@ -445,7 +454,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
           const int r = __shfl_sync(~0u, nd.r, b), p = __shfl_sync(~0u, my, b);
           leaf_range(p + 1, r - p);
         }
-        if constexpr (MODE == 0) { if (cap > 0 && !__any_sync(~0u, alive)) break; }
+        if (capped && !__any_sync(~0u, alive)) break;
         const uint32_t b0 = __ballot_sync(~0u, in0), b1 = __ballot_sync(~0u, in1);
         if (in0) stack[nlist + __popc(b0 & lt)] = nd.c0;
         if (in1) stack[nlist + __popc(b0) + __popc(b1 & lt)] = nd.c1;
@@ -775,11 +784,11 @@ arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s
   if (const char* v = getenv("ARBX_PACKET_ALPHA")) alpha = (float)atof(v);
   const int n = (int)ix->n;
   if (a.pass == 1)
-    spatial_kernel<PK, QK, 1><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, mode, alpha);
+    spatial_kernel<PK, QK, 1><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, a.stop_fill, mode, alpha);
   else if (a.pass == 2)
-    spatial_kernel<PK, QK, 2><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, mode, alpha);
+    spatial_kernel<PK, QK, 2><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, 0, mode, alpha);
   else
-    spatial_kernel<PK, QK, 0><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, a.cap, nullptr, mode, alpha);
+    spatial_kernel<PK, QK, 0><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, a.cap, nullptr, 0, mode, alpha);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }

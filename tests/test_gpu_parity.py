@@ -449,3 +449,31 @@ def test_run_to_run_determinism(arbx):
             ref = cur
         else:
             assert all(torch.equal(a, b) for a, b in zip(ref, cur))
+
+
+@pytest.mark.parametrize("traversal", ["thread", "packet", None])
+def test_spatial_upto(arbx, orc, monkeypatch, traversal):
+    """Capped storage query (PAPER.md:L174 early exit from a storing callback)."""
+    from oracle import compare as cmp
+    if traversal:
+        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    prims = dg.uniform_points(8000, 3, 81)
+    q = dg.sphere_queries(dg.uniform_points(5000, 3, 82), 0.08)
+    o = orc.spatial(prims, dg.POINT, q, dg.SPHERE)
+    ix = arbx.Index(_dev(prims), dg.POINT)
+    for limit in (1, 6, 100, 10_000):
+        off, idx = ix.query_spatial_upto(_dev(q), limit, dg.SPHERE)
+        cmp.compare_spatial_upto(len(prims), o, (_np(off), _np(idx)), limit, f"spatial_upto {limit} {traversal}")
+        c = _np(ix.query_count(_dev(q), dg.SPHERE, limit=limit))
+        assert np.array_equal(c, np.diff(_np(off)))                 # same capped counts
+    off, idx = ix.query_spatial_upto(_dev(q), 10_000, dg.SPHERE)        # a cap nobody reaches = the full query
+    cmp.compare_spatial(len(prims), o, (_np(off), _np(idx)), "spatial_upto unlimited")
+    ix.close()
+    boxes = dg.uniform_boxes(6000, 3, 83, 0.03)
+    qb = dg.uniform_boxes(3000, 3, 84, 0.05)
+    ob = orc.spatial(boxes, dg.BOX, qb, dg.BOX)
+    ixb = arbx.Index(_dev(boxes), dg.BOX)
+    off, idx = ixb.query_spatial_upto(_dev(qb), 4, dg.BOX)
+    cmp.compare_spatial_upto(len(boxes), ob, (_np(off), _np(idx)), 4, "spatial_upto boxes")
+    assert np.array_equal(np.diff(_np(off)), np.minimum(np.diff(ob[0]), 4))
+    ixb.close()
