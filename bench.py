@@ -371,6 +371,20 @@ def main():
                 b.record(stream)
             torch.cuda.synchronize()
             extras[f"count_upto_{limit}_qps"] = round(nq / a.elapsed_time(b) * 1e3, 1)
+        if pk == 0 and qk == 2 and cfg["r"]:
+            # NEXT-2 self-join over the primitives themselves with the workload's radius (device-timed)
+            poff = torch.empty(n + 1, dtype=torch.int32, device=dev)
+            _, ptotal = arbx.arbx_query_pairs(hx, float(cfg["r"]), poff, None, 0, stream)
+            pidx = torch.empty(max(ptotal, 1), dtype=torch.int32, device=dev)
+            for rep in range(3):
+                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                arbx.arbx_query_pairs(hx, float(cfg["r"]), poff, pidx, pidx.numel(), stream)
+                b.record(stream)
+            torch.cuda.synchronize()
+            extras["self_join_pairs"] = int(ptotal)
+            extras["self_join_prims_per_s"] = round(n / a.elapsed_time(b) * 1e3, 1)
+            del poff, pidx
         arbx.arbx_destroy(hx, stream)
     torch.cuda.synchronize()
 

@@ -124,6 +124,16 @@ ARBX_API arbx_status arbx_query_spatial_upto(arbx_handle h, const float* queries
                                     int32_t limit, int32_t* offsets, int32_t* indices,
                                     int64_t indices_capacity, int64_t* total_host, arbx_stream stream);
 
+/* Self-join / pair search over the index's own POINT primitives ("special
+ * traversal algorithm when searching for pairs of objects"): every unordered
+ * pair {i,j}, i != j, with ||x_i - x_j|| <= radius (closed) is reported EXACTLY ONCE, either as
+ * j in row i or as i in row j (which of the two is unspecified).  offsets: DEVICE int32[n+1],
+ * rows in the caller's primitive order; indices / capacity / total_host / errors as in
+ * arbx_query_spatial.  Half traversal: a query only visits subtrees after its own leaf.
+ * ARBX_ERR_UNSUPPORTED for BOX / SPHERE primitives.                                           */
+ARBX_API arbx_status arbx_query_pairs(arbx_handle h, float radius, int32_t* offsets, int32_t* indices,
+                             int64_t indices_capacity, int64_t* total_host, arbx_stream stream);
+
 /* k nearest primitives to each query point ("a pair of a query point and a
  * number of neighbors"; L79 distance to the stored geometry: point ||x-y||, box point-box
  * distance (0 inside), sphere max(0,||y-c||-R)).  qpoints: DEVICE nq*dim.  One k per call,

@@ -138,3 +138,25 @@ def compare_spatial_upto(n: int, orc, got, limit: int, what: str = "") -> None:
     extra = ~np.isin(kg, ko, assume_unique=True)
     assert not extra.any(), f"{what}: {int(extra.sum())} reported pairs are not matches"
     compare_counts_upto(orc, np.diff(np.asarray(g_off, dtype=np.int64)), limit, what)
+
+
+def compare_pairs(n: int, orc, got, what: str = "") -> dict:
+    """Self-join (PAPER.md:L305): orc = oracle.spatial(points, POINT, (points, r), SPHERE), i.e.
+    the full symmetric neighbour lists INCLUDING the self matches; got = (offsets[n+1], indices)
+    where every unordered pair {i,j}, i != j, within r must appear exactly once in either row."""
+    o_off, o_idx, o_band = orc
+    g_off, g_idx = got
+    check_csr_format(g_off, g_idx, n, n)
+    rows_o = np.repeat(np.arange(n, dtype=np.int64), np.diff(np.asarray(o_off, dtype=np.int64)))
+    oi = np.asarray(o_idx, dtype=np.int64)
+    up = rows_o < oi                                        # each unordered pair once, self matches dropped
+    ko = rows_o[up] * n + oi[up]
+    sure = ko[np.asarray(o_band)[up] == 0]
+    rows_g = np.repeat(np.arange(n, dtype=np.int64), np.diff(np.asarray(g_off, dtype=np.int64)))
+    gi = np.asarray(g_idx, dtype=np.int64)
+    assert not np.any(rows_g == gi), f"{what}: a primitive is paired with itself"
+    kg = np.sort(np.minimum(rows_g, gi) * n + np.maximum(rows_g, gi))
+    assert np.all(np.diff(kg) > 0), f"{what}: an unordered pair is reported more than once"
+    assert np.isin(sure, kg, assume_unique=True).all(), f"{what}: a sure pair is missing"
+    assert np.isin(kg, ko, assume_unique=True).all(), f"{what}: a reported pair is not within the radius"
+    return dict(pairs=int(len(kg)), sure=int(len(sure)))

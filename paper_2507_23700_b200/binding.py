@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libarbx.so")
 
 EXPORTS = (
     "arbx_build", "arbx_destroy", "arbx_size", "arbx_bounds", "arbx_query_count",
-    "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_spatial_upto", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
+    "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_spatial_upto", "arbx_query_pairs", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
     "arbx_launch_count", "arbx_profile_enable", "arbx_profile_num_kernels",
     "arbx_profile_kernel_name", "arbx_profile_read", "arbx_status_string", "arbx_last_error",
 )
@@ -57,6 +57,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_query_count_upto.argtypes = [vp, vp, i64, i32, i32, vp, vp]
         L.arbx_query_spatial.argtypes = [vp, vp, i64, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.arbx_query_spatial_upto.argtypes = [vp, vp, i64, i32, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.arbx_query_pairs.argtypes = [vp, ctypes.c_float, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.arbx_query_knn.argtypes = [vp, vp, i64, i32, vp, vp, vp]
         L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
         L.arbx_debug_validate.argtypes = [vp, ctypes.POINTER(i64), vp]
@@ -71,7 +72,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_status_string.restype = ctypes.c_char_p
         L.arbx_status_string.argtypes = [i32]
         L.arbx_last_error.restype = ctypes.c_char_p
-        for name in EXPORTS[:11]:
+        for name in EXPORTS[:12]:
             getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -163,6 +164,16 @@ def arbx_query_spatial_upto(handle: int, queries: torch.Tensor, nq: int, qkind: 
                                        ctypes.byref(total), _stream(stream))
     if st not in (OK, ERR_CAPACITY):
         raise ArbxError(st, "arbx_query_spatial_upto")
+    return st, total.value
+
+
+def arbx_query_pairs(handle: int, radius: float, offsets: torch.Tensor, indices, capacity: int, stream=None):
+    """Returns (status, total); ERR_CAPACITY is returned, not raised."""
+    total = ctypes.c_int64()
+    st = lib().arbx_query_pairs(handle, radius, offsets.data_ptr(), 0 if indices is None else indices.data_ptr(),
+                                capacity, ctypes.byref(total), _stream(stream))
+    if st not in (OK, ERR_CAPACITY):
+        raise ArbxError(st, "arbx_query_pairs")
     return st, total.value
 
 
@@ -278,6 +289,15 @@ class Index:
         indices = torch.empty(max(nq * limit, 1), dtype=torch.int32, device=self.device)
         _, total = arbx_query_spatial_upto(self.handle, queries, nq, qkind, limit, offsets, indices,
                                            indices.numel(), stream)
+        return offsets, indices[:total]
+
+    def query_pairs(self, radius: float, stream=None):
+        """Self-join: CSR (offsets int32[n+1], indices) holding every unordered pair within radius once."""
+        n = self.size()
+        offsets = torch.empty(n + 1, dtype=torch.int32, device=self.device)
+        _, total = arbx_query_pairs(self.handle, radius, offsets, None, 0, stream)
+        indices = torch.empty(max(total, 1), dtype=torch.int32, device=self.device)
+        arbx_query_pairs(self.handle, radius, offsets, indices, indices.numel(), stream)
         return offsets, indices[:total]
 
     def query_knn(self, qpoints: torch.Tensor, k: int, want_distances: bool = True, stream=None):

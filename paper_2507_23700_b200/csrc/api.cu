@@ -132,6 +132,19 @@ __global__ void fill_knn_empty_kernel(int32_t* idx, float* dist, int64_t n) {
   }
 }
 
+// self-join queries: query i = (point i, radius) in the caller's order; order[t] = caller's
+// index of the leaf at sorted position t (so no query sort is needed: tree order IS the order)
+__global__ void self_queries_kernel(const float* __restrict__ leaves, int64_t n, int D, int LW, float radius,
+                                    float* __restrict__ queries, uint32_t* __restrict__ order) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const float* lf = leaves + t * LW;
+  const uint32_t idx = __float_as_uint(lf[D]) & ~LEAF_END;
+  for (int a = 0; a < D; ++a) queries[(int64_t)idx * (D + 1) + a] = lf[a];
+  queries[(int64_t)idx * (D + 1) + D] = radius;
+  order[t] = idx;
+}
+
 }  // namespace arbx
 
 using namespace arbx;
@@ -220,7 +233,7 @@ static arbx_status count_impl(arbx_handle h, const float* queries, int64_t nq, a
 
 static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind, int32_t limit,
                                 int32_t* offsets, int32_t* indices, int64_t indices_capacity,
-                                int64_t* total_host, arbx_stream stream);
+                                int64_t* total_host, arbx_stream stream, float self_radius = -1.f);
 
 arbx_status arbx_query_spatial(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
                                int32_t* offsets, int32_t* indices, int64_t indices_capacity,
@@ -235,10 +248,19 @@ arbx_status arbx_query_spatial_upto(arbx_handle h, const float* queries, int64_t
   return spatial_impl(h, queries, nq, qkind, limit, offsets, indices, indices_capacity, total_host, stream);
 }
 
+arbx_status arbx_query_pairs(arbx_handle h, float radius, int32_t* offsets, int32_t* indices,
+                             int64_t indices_capacity, int64_t* total_host, arbx_stream stream) {
+  if (!h || !(radius >= 0.f)) { set_error("arbx_query_pairs: invalid argument"); return ARBX_ERR_INVALID_ARG; }
+  if (h->ix.kind != KIND_POINT) { set_error("arbx_query_pairs: POINT primitives only"); return ARBX_ERR_UNSUPPORTED; }
+  return spatial_impl(h, nullptr, h->ix.n, ARBX_SPHERE, 0, offsets, indices, indices_capacity, total_host, stream, radius);
+}
+
 static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind, int32_t limit,
                                 int32_t* offsets, int32_t* indices, int64_t indices_capacity,
-                                int64_t* total_host, arbx_stream stream) {
-  if (!h || nq < 0 || bad_kind((int)qkind) || !offsets || (nq > 0 && !queries) || indices_capacity < 0) {
+                                int64_t* total_host, arbx_stream stream, float self_radius) {
+  const bool self = self_radius >= 0.f;
+  if (self && h) nq = h->ix.n;
+  if (!h || nq < 0 || bad_kind((int)qkind) || !offsets || (nq > 0 && !queries && !self) || indices_capacity < 0) {
     set_error("arbx_query_spatial: invalid argument");
     return ARBX_ERR_INVALID_ARG;
   }
@@ -253,7 +275,17 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
   Scratch<uint32_t> order;
   Scratch<int32_t> counts, rows;
   Scratch<long long> total_dev;   // [0] total, [1] number of queries with more than `cap` matches
-  ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
+  Scratch<float> selfq;
+  if (self) {
+    ARBX_TRY(selfq.alloc((size_t)nq * (ix->dim + 1), s));
+    ARBX_TRY(order.alloc((size_t)nq, s));
+    self_queries_kernel<<<(unsigned)((nq + 255) / 256), 256, 0, s>>>(ix->leaves, nq, ix->dim, leaf_width(KIND_POINT, ix->dim),
+                                                                  self_radius, selfq.p, order.p);
+    ARBX_LAUNCH_CHECK();
+    queries = selfq.p;
+  } else {
+    ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
+  }
   ARBX_TRY(counts.alloc((size_t)nq, s));
   ARBX_TRY(total_dev.alloc(2, s));
   ARBX_CUDA(cudaMemsetAsync(total_dev.p, 0, 2 * sizeof(long long), s));
@@ -271,6 +303,7 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
                 reinterpret_cast<int*>(total_dev.p + 1), cap ? 2 : 0};
   // capped storage query: capped count (early exit) -> scan -> fill that stops at each count
   if (limit > 0) a.cap = limit;
+  a.self = self ? 1 : 0;
   if (cap) {
     ARBX_TRY(rows.alloc((size_t)nq * cap, s));
     a.rows = rows.p;

@@ -131,6 +131,7 @@ struct SpatialArgs {
   int32_t* counts; const int32_t* offsets; int32_t* indices;
   int32_t* rows; int cap; int* overflow; int pass;
   int stop_fill = 0;   // pass 1 only: query q stops after counts[q] hits (capped storage query)
+  int self = 0;        // self-join: query t is the leaf at sorted position t; report later positions only
 };
 using spatial_fn = arbx_status (*)(const Index*, const SpatialArgs&, cudaStream_t);
 using knn_fn = arbx_status (*)(const Index*, const float* qpoints, int64_t nq, int k,

@@ -143,10 +143,27 @@ __device__ __forceinline__ bool hits_prim(const Query<QK>& q, const float* p) {
 // instead of 32 divergent ones, control flow is uniform, and the stack is one short array
 // per warp in shared memory.  The leaf test is per lane and exact, so the result is the same
 // set as one-query-per-thread traversal.
-template <int PK, int QK, bool FILL>
+struct NodeX { float v[4 * D]; int32_t c0, c1, l, r; };
+
+__device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, int32_t ref, NodeX& nd) {
+  const float4* p = nodes + (int64_t)ref * (D + 1);
+#pragma unroll
+  for (int e = 0; e < D; ++e) {
+    float4 t = __ldg(p + e);
+    nd.v[4 * e] = t.x; nd.v[4 * e + 1] = t.y; nd.v[4 * e + 2] = t.z; nd.v[4 * e + 3] = t.w;
+  }
+  float4 t = __ldg(p + D);
+  nd.c0 = __float_as_int(t.x); nd.c1 = __float_as_int(t.y);
+  nd.l = __float_as_int(t.z); nd.r = __float_as_int(t.w);
+}
+
+// SELF (self-join, queries = the index's own primitives in tree order): query number `tpos` is
+// the leaf at sorted position tpos; only primitives at LATER positions are reported, so every
+// unordered pair appears once, and subtrees that end at or before tpos are skipped.
+template <int PK, int QK, bool FILL, bool SELF>
 __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes, const float4* __restrict__ leaves,
                                                const int32_t* __restrict__ root, const Query<QK>& q,
-                                               int32_t* __restrict__ out, int limit, int stop) {
+                                               int32_t* __restrict__ out, int limit, int stop, int tpos) {
   int cnt = 0;
   int32_t stack[STACK_DEPTH];
   int sp = 0;
@@ -154,10 +171,11 @@ __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes,
   int32_t ref = __ldg(root);
   for (;;) {   // while-while: descend to a leaf range in every lane, then scan together
     while (ref >= 0) {
-      Node nd;
-      load_node(nodes, ref, nd);
-      const bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
-      const bool h1 = hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D);
+      NodeX nd;
+      load_node_x(nodes, ref, nd);
+      bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
+      bool h1 = hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D);
+      if constexpr (SELF) { h0 = h0 && ref > tpos; h1 = h1 && nd.r > tpos; }   // child ranges [l,ref], [ref+1,r]
       if (h0) {
         ref = nd.c0;
         if (h1) stack[sp++] = nd.c1;
@@ -172,7 +190,7 @@ __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes,
     for (;; ++j) {
       Leaf<PK> lf;
       load_leaf<PK>(leaves, j, lf);
-      if (hits_prim<QK, PK>(q, lf.v)) {
+      if ((!SELF || j > tpos) && hits_prim<QK, PK>(q, lf.v)) {
         if constexpr (FILL) { if (cnt < limit) out[cnt] = (int32_t)(lf.idx & ~LEAF_END); }
         ++cnt;
         if (cnt >= stop) return cnt;   // capped query: early exit
@@ -280,24 +298,10 @@ __device__ __forceinline__ bool joint_hits_box(const Joint<QK>& J, const float* 
   }
 }
 
-struct NodeX { float v[4 * D]; int32_t c0, c1, l, r; };
-
-__device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, int32_t ref, NodeX& nd) {
-  const float4* p = nodes + (int64_t)ref * (D + 1);
-#pragma unroll
-  for (int e = 0; e < D; ++e) {
-    float4 t = __ldg(p + e);
-    nd.v[4 * e] = t.x; nd.v[4 * e + 1] = t.y; nd.v[4 * e + 2] = t.z; nd.v[4 * e + 3] = t.w;
-  }
-  float4 t = __ldg(p + D);
-  nd.c0 = __float_as_int(t.x); nd.c1 = __float_as_int(t.y);
-  nd.l = __float_as_int(t.z); nd.r = __float_as_int(t.w);
-}
-
 // MODE 0: count.  MODE 1: fill the CSR slices (offsets known); with cap > 0 the queries whose
 // count is <= cap are skipped (their rows were stored by MODE 2 and are copied by
 // compact_rows).  MODE 2: count AND store the first `cap` hits of query q in rows[q*cap ..].
-template <int PK, int QK, int MODE>
+template <int PK, int QK, int MODE, bool SELF>
 __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ nodes,
                                                      const float4* __restrict__ leaves,
                                                      const int32_t* __restrict__ root, int n,
@@ -347,8 +351,8 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   // mode 0: per-warp choice; 1: always one query per lane; 2: always packet
   if (mode == 1 || (mode == 0 && !warp_coherent<QK>(q, valid, alpha))) {
     int c = 0;
-    if (alive) c = thread_traverse<PK, QK, FILL>(nodes, leaves, root, q, FILL ? indices + base64 : nullptr, limit,
-                                                  capped ? limit : INT32_MAX);
+    if (alive) c = thread_traverse<PK, QK, FILL, SELF>(nodes, leaves, root, q, FILL ? indices + base64 : nullptr, limit,
+                                                        capped ? limit : INT32_MAX, (int)t);
     if constexpr (MODE != 1) {
       if (valid) counts[qi] = c;
       if constexpr (MODE == 2) { if (c > cap) atomicAdd(overflow, 1); }
@@ -397,7 +401,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
         todo &= todo - 1;
         Leaf<PK> lf;
         load_leaf<PK>(leaves, first + j0 + b, lf);
-        const bool hit = alive && hits_prim<QK, PK>(q, lf.v);
+        const bool hit = alive && (!SELF || first + j0 + b > (int)t) && hits_prim<QK, PK>(q, lf.v);
         if constexpr (FILL) {
           const uint32_t full = __ballot_sync(~0u, pend == FS);
           if (full) flush(full);
@@ -436,8 +440,12 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
         bool in0 = false, in1 = false, lf0 = false, lf1 = false;
         if (my >= 0) {
           load_node_x(nodes, my, nd);
-          const bool h0 = joint_hits_box<QK>(J, nd.v, nd.v + D);
-          const bool h1 = joint_hits_box<QK>(J, nd.v + 2 * D, nd.v + 3 * D);
+          bool h0 = joint_hits_box<QK>(J, nd.v, nd.v + D);
+          bool h1 = joint_hits_box<QK>(J, nd.v + 2 * D, nd.v + 3 * D);
+          if constexpr (SELF) {   // the warp's smallest query position is its first lane's
+            const int tmin = (int)(t - lane);
+            h0 = h0 && my > tmin; h1 = h1 && nd.r > tmin;
+          }
           in0 = h0 && nd.c0 >= 0; lf0 = h0 && nd.c0 < 0;
           in1 = h1 && nd.c1 >= 0; lf1 = h1 && nd.c1 < 0;
         }
@@ -771,7 +779,7 @@ inline int traversal_mode() {
 }
 
 // ---- host dispatch ------------------------------------------------------------------------------------
-template <int PK, int QK>
+template <int PK, int QK, bool SELF = false>
 arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s) {
   const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);
   const float4* nodes = reinterpret_cast<const float4*>(ix->nodes);
@@ -784,11 +792,11 @@ arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s
   if (const char* v = getenv("ARBX_PACKET_ALPHA")) alpha = (float)atof(v);
   const int n = (int)ix->n;
   if (a.pass == 1)
-    spatial_kernel<PK, QK, 1><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, a.stop_fill, mode, alpha);
+    spatial_kernel<PK, QK, 1, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, a.stop_fill, mode, alpha);
   else if (a.pass == 2)
-    spatial_kernel<PK, QK, 2><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, 0, mode, alpha);
+    spatial_kernel<PK, QK, 2, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, 0, mode, alpha);
   else
-    spatial_kernel<PK, QK, 0><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, a.cap, nullptr, 0, mode, alpha);
+    spatial_kernel<PK, QK, 0, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, a.cap, nullptr, 0, mode, alpha);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
@@ -803,6 +811,7 @@ arbx_status spatial_pk(const Index* ix, const SpatialArgs& a, cudaStream_t s) {
 }
 
 arbx_status spatial_entry(const Index* ix, const SpatialArgs& a, cudaStream_t s) {
+  if (a.self) return spatial_launch<KIND_POINT, KIND_SPHERE, true>(ix, a, s);   // api.cu guarantees POINT prims
   switch (ix->kind) {
     case KIND_POINT: return spatial_pk<KIND_POINT>(ix, a, s);
     case KIND_BOX: return spatial_pk<KIND_BOX>(ix, a, s);

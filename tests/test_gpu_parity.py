@@ -477,3 +477,38 @@ def test_spatial_upto(arbx, orc, monkeypatch, traversal):
     cmp.compare_spatial_upto(len(boxes), ob, (_np(off), _np(idx)), 4, "spatial_upto boxes")
     assert np.array_equal(np.diff(_np(off)), np.minimum(np.diff(ob[0]), 4))
     ixb.close()
+
+
+# ---- NEXT-2: self-join / pair search ------------------------------------------------------
+@pytest.mark.parametrize("traversal", ["thread", "packet", None])
+@pytest.mark.parametrize("D", [2, 3, 5])
+def test_query_pairs(arbx, orc, monkeypatch, traversal, D):
+    from oracle import compare as cmp
+    if traversal:
+        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    n = 6000
+    p = dg.uniform_points(n, D, 90 + D)
+    p[100:140] = p[100]                                      # a clump of duplicates: distance 0 pairs
+    r = 0.5 * (12.0 / n) ** (1.0 / D)
+    o = orc.spatial(p, dg.POINT, dg.sphere_queries(p, r), dg.SPHERE)
+    ix = arbx.Index(_dev(p), dg.POINT)
+    off, idx = ix.query_pairs(r)
+    st = cmp.compare_pairs(n, o, (_np(off), _np(idx)), f"pairs D={D} {traversal}")
+    assert st["pairs"] >= 40 * 39 // 2
+    off0, idx0 = ix.query_pairs(0.0)                         # r = 0: exactly the duplicate pairs
+    assert idx0.numel() == 40 * 39 // 2
+    ix.close()
+
+
+def test_query_pairs_lattice_and_errors(arbx):
+    g = 7
+    p = dg.lattice_points(g, 3)
+    ix = arbx.Index(_dev(p), dg.POINT)
+    off, idx = ix.query_pairs(1.0)
+    assert idx.numel() == 3 * g * g * (g - 1)                # axis-neighbour pairs of a g^3 lattice, once each
+    ix.close()
+    b = arbx.Index(_dev(dg.uniform_boxes(100, 3, 1, 0.1)), dg.BOX)
+    with pytest.raises(arbx.ArbxError) as e:
+        b.query_pairs(0.1)
+    assert e.value.status == arbx.ERR_UNSUPPORTED
+    b.close()

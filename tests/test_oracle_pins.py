@@ -282,3 +282,30 @@ def test_capped_count_comparator_is_min_of_definition(orc):
         cmp.compare_counts_upto(o, np.minimum(rows, limit), limit)
     with pytest.raises(AssertionError):
         cmp.compare_counts_upto(o, np.minimum(rows, 6 + 1), 6)
+
+
+def test_pair_comparator_closed_form(orc):
+    """compare_pairs on a lattice: r = 1.2 gives exactly the 3 g^2 (g-1) axis-neighbour pairs (all
+    clear of the tolerance band); it rejects a duplicated pair, a self pair and a missing pair."""
+    from oracle import compare as cmp
+    from paper_2507_23700_b200 import datagen as dg
+    g = 4
+    p = dg.lattice_points(g, 3)
+    n = len(p)
+    o = orc.spatial(p, dg.POINT, dg.sphere_queries(p, 1.2), dg.SPHERE)
+    assert not o[2].any()
+    rows = np.repeat(np.arange(n), np.diff(o[0]))
+    up = rows < o[1]
+    a, b = rows[up], o[1][up]
+    assert len(a) == 3 * g * g * (g - 1)
+    order = np.argsort(a, kind="stable")
+    off = np.concatenate([[0], np.cumsum(np.bincount(a, minlength=n))])
+    good = (off, b[order].astype(np.int32))
+    assert cmp.compare_pairs(n, o, good)["pairs"] == len(a)
+    flipped = (np.concatenate([[0], np.cumsum(np.bincount(b, minlength=n))]), a[np.argsort(b, kind="stable")].astype(np.int32))
+    cmp.compare_pairs(n, o, flipped)                          # the other endpoint may own the pair
+    both = (o[0], o[1])                                       # full symmetric lists: pairs twice + self
+    with pytest.raises(AssertionError):
+        cmp.compare_pairs(n, o, both)
+    with pytest.raises(AssertionError):
+        cmp.compare_pairs(n, o, (np.maximum(off - (off > 0), 0), good[1][1:]))   # one pair dropped
