@@ -382,6 +382,15 @@ def main():
                 arbx.arbx_query_pairs(hx, float(cfg["r"]), poff, pidx, pidx.numel(), stream)
                 b.record(stream)
             torch.cuda.synchronize()
+            lab = torch.empty(n, dtype=torch.int32, device=dev)
+            for rep in range(2):
+                c = torch.cuda.Event(enable_timing=True); d = torch.cuda.Event(enable_timing=True)
+                c.record(stream)
+                arbx.arbx_dbscan(hx, float(cfg["r"]), 8, lab, stream)
+                d.record(stream)
+            torch.cuda.synchronize()
+            extras["dbscan_minpts8_prims_per_s"] = round(n / c.elapsed_time(d) * 1e3, 1)
+            extras["dbscan_clusters"] = int((lab == torch.arange(n, device=dev, dtype=torch.int32)).sum())
             extras["self_join_pairs"] = int(ptotal)
             extras["self_join_prims_per_s"] = round(n / a.elapsed_time(b) * 1e3, 1)
             del poff, pidx

@@ -134,6 +134,15 @@ ARBX_API arbx_status arbx_query_spatial_upto(arbx_handle h, const float* queries
 ARBX_API arbx_status arbx_query_pairs(arbx_handle h, float radius, int32_t* offsets, int32_t* indices,
                              int64_t indices_capacity, int64_t* total_host, arbx_stream stream);
 
+/* DBSCAN over the index's own POINT primitives (PAPER.md:L251-257 FDBSCAN: density clustering
+ * on the search index; L274-277 dbscan(space, points, eps, minPts) -> labels, -1 = noise;
+ * SURVEY.md NEXT-3).  A point is a CORE point iff at least min_pts primitives (itself included)
+ * lie within eps (closed).  Core points within eps of each other share a cluster; a non-core
+ * point within eps of a core point is a BORDER point of (any) one such cluster; all other
+ * points are noise.  labels: DEVICE int32[n]; labels[i] = the smallest caller index of a core
+ * point of i's cluster, or -1 for noise.  Asynchronous on `stream`.  POINT primitives only.   */
+ARBX_API arbx_status arbx_dbscan(arbx_handle h, float eps, int32_t min_pts, int32_t* labels, arbx_stream stream);
+
 /* k nearest primitives to each query point ("a pair of a query point and a
  * number of neighbors"; L79 distance to the stored geometry: point ||x-y||, box point-box
  * distance (0 inside), sphere max(0,||y-c||-R)).  qpoints: DEVICE nq*dim.  One k per call,

@@ -155,3 +155,33 @@ def default_cell(prims, pkind: int, mode: str, r: float | None = None, per_cell:
     if mode == "spatial" and r is not None and r > 0:
         return max(float(r), 0.5 * occ)
     return occ
+
+
+def dbscan(points, eps: float, min_pts: int):
+    """Textbook DBSCAN on the brute-force /
+    grid neighbour lists of this oracle.  A point is core iff >= min_pts points (itself
+    included) lie within eps (closed); clusters are the connected components of the core
+    points under "within eps"; a non-core point within eps of a core point is a border point
+    and may belong to ANY adjacent core's cluster; the rest is noise.
+    Returns (core bool[n], comp int[n] (component id of core points, -1 otherwise),
+             allowed: list of sets of component ids a border point may take (empty = noise),
+             band_any: True if some pair sits in the 1e-6 tolerance band (then compare loosely))."""
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import connected_components
+    points = _f32(points)
+    n = points.shape[0]
+    q = np.concatenate([points, np.full((n, 1), eps, dtype=np.float32)], axis=1)
+    grid = Grid(points, POINT, max(float(eps), 1e-6)) if n > 20000 else None
+    off, idx, band = spatial(points, POINT, q, SPHERE, grid)
+    counts = np.diff(off)
+    core = counts >= min_pts
+    rows = np.repeat(np.arange(n), counts)
+    keep = core[rows] & core[idx]
+    g = csr_matrix((np.ones(int(keep.sum()), dtype=np.int8), (rows[keep], idx[keep])), shape=(n, n))
+    _, lab = connected_components(g, directed=False)
+    comp = np.where(core, lab, -1)
+    allowed = [set() for _ in range(n)]
+    nb = (~core[rows]) & core[idx]
+    for r, c in zip(rows[nb], idx[nb]):
+        allowed[r].add(int(comp[c]))
+    return core, comp, allowed, bool(band.any())

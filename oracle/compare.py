@@ -160,3 +160,28 @@ def compare_pairs(n: int, orc, got, what: str = "") -> dict:
     assert np.isin(sure, kg, assume_unique=True).all(), f"{what}: a sure pair is missing"
     assert np.isin(kg, ko, assume_unique=True).all(), f"{what}: a reported pair is not within the radius"
     return dict(pairs=int(len(kg)), sure=int(len(sure)))
+
+
+def compare_dbscan(orc, labels, what: str = "") -> dict:
+    """orc = oracle.dbscan(...); labels = int32[n] with -1 = noise.  The core partition must
+    be the same up to renaming; a border point must carry the label of one of its adjacent
+    cores' clusters; noise must be -1.  (Use inputs without band pairs: orc[3] False.)"""
+    core, comp, allowed, band_any = orc
+    assert not band_any, f"{what}: choose eps so that no pair sits in the tolerance band"
+    labels = np.asarray(labels, dtype=np.int64)
+    n = len(core)
+    assert labels.shape == (n,)
+    lc, cc = labels[core], comp[core]
+    assert np.all(lc >= 0), f"{what}: a core point is labelled noise"
+    # bijection between oracle components and reported labels on the core points
+    pairs = np.unique(np.stack([cc, lc], axis=1), axis=0)
+    assert len(np.unique(pairs[:, 0])) == len(pairs) == len(np.unique(pairs[:, 1])), f"{what}: core partition differs"
+    to_label = {int(c): int(l) for c, l in pairs}
+    nborder = 0
+    for i in np.nonzero(~core)[0]:
+        if allowed[i]:
+            nborder += 1
+            assert int(labels[i]) in {to_label[c] for c in allowed[i]}, f"{what}: border point {i} has a foreign label"
+        else:
+            assert labels[i] == -1, f"{what}: noise point {i} has label {labels[i]}"
+    return dict(clusters=len(pairs), core=int(core.sum()), border=nborder, noise=int(n - core.sum() - nborder))

@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libarbx.so")
 
 EXPORTS = (
     "arbx_build", "arbx_destroy", "arbx_size", "arbx_bounds", "arbx_query_count",
-    "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_spatial_upto", "arbx_query_pairs", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
+    "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_spatial_upto", "arbx_query_pairs", "arbx_dbscan", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
     "arbx_launch_count", "arbx_profile_enable", "arbx_profile_num_kernels",
     "arbx_profile_kernel_name", "arbx_profile_read", "arbx_status_string", "arbx_last_error",
 )
@@ -58,6 +58,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_query_spatial.argtypes = [vp, vp, i64, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.arbx_query_spatial_upto.argtypes = [vp, vp, i64, i32, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.arbx_query_pairs.argtypes = [vp, ctypes.c_float, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.arbx_dbscan.argtypes = [vp, ctypes.c_float, i32, vp, vp]
         L.arbx_query_knn.argtypes = [vp, vp, i64, i32, vp, vp, vp]
         L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
         L.arbx_debug_validate.argtypes = [vp, ctypes.POINTER(i64), vp]
@@ -72,7 +73,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_status_string.restype = ctypes.c_char_p
         L.arbx_status_string.argtypes = [i32]
         L.arbx_last_error.restype = ctypes.c_char_p
-        for name in EXPORTS[:12]:
+        for name in EXPORTS[:13]:
             getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -175,6 +176,10 @@ def arbx_query_pairs(handle: int, radius: float, offsets: torch.Tensor, indices,
     if st not in (OK, ERR_CAPACITY):
         raise ArbxError(st, "arbx_query_pairs")
     return st, total.value
+
+
+def arbx_dbscan(handle: int, eps: float, min_pts: int, labels: torch.Tensor, stream=None) -> None:
+    _check(lib().arbx_dbscan(handle, eps, min_pts, _ptr(labels), _stream(stream)), "arbx_dbscan")
 
 
 def arbx_query_knn(handle: int, qpoints: torch.Tensor, nq: int, k: int, indices: torch.Tensor,
@@ -299,6 +304,12 @@ class Index:
         indices = torch.empty(max(total, 1), dtype=torch.int32, device=self.device)
         arbx_query_pairs(self.handle, radius, offsets, indices, indices.numel(), stream)
         return offsets, indices[:total]
+
+    def dbscan(self, eps: float, min_pts: int, stream=None) -> torch.Tensor:
+        """labels int32[n]: smallest core index of the point's cluster, -1 = noise."""
+        labels = torch.empty(self.size(), dtype=torch.int32, device=self.device)
+        arbx_dbscan(self.handle, eps, min_pts, labels, stream)
+        return labels
 
     def query_knn(self, qpoints: torch.Tensor, k: int, want_distances: bool = True, stream=None):
         nq = self._nq(qpoints, POINT)

@@ -145,6 +145,24 @@ __global__ void self_queries_kernel(const float* __restrict__ leaves, int64_t n,
   order[t] = idx;
 }
 
+// ---- DBSCAN glue (arbx_dbscan) ------------------------------------------------------------------
+__global__ void dbscan_init_kernel(const int32_t* __restrict__ counts, int min_pts, int64_t n, int32_t* __restrict__ uf) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) uf[i] = counts[i] >= min_pts ? (int32_t)i : -1;     // core points start as their own cluster
+}
+// label = smallest core index of the cluster; a border point takes the cluster of the core point
+// it remembered; everything else is noise (-1)
+__global__ void dbscan_labels_kernel(const int32_t* __restrict__ uf, int64_t n, int32_t* __restrict__ labels) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int32_t x = uf[i];
+  if (x == -1) { labels[i] = -1; return; }
+  if (x <= -2) x = -2 - x;                     // border: follow the remembered core point
+  else x = (int32_t)i;
+  for (int32_t p = uf[x]; p != x; p = uf[x]) x = p;   // the forest is final here: plain root walk
+  labels[i] = x;
+}
+
 }  // namespace arbx
 
 using namespace arbx;
@@ -253,6 +271,43 @@ arbx_status arbx_query_pairs(arbx_handle h, float radius, int32_t* offsets, int3
   if (!h || !(radius >= 0.f)) { set_error("arbx_query_pairs: invalid argument"); return ARBX_ERR_INVALID_ARG; }
   if (h->ix.kind != KIND_POINT) { set_error("arbx_query_pairs: POINT primitives only"); return ARBX_ERR_UNSUPPORTED; }
   return spatial_impl(h, nullptr, h->ix.n, ARBX_SPHERE, 0, offsets, indices, indices_capacity, total_host, stream, radius);
+}
+
+arbx_status arbx_dbscan(arbx_handle h, float eps, int32_t min_pts, int32_t* labels, arbx_stream stream) {
+  if (!h || !(eps >= 0.f) || min_pts < 1 || (h->ix.n > 0 && !labels)) {
+    set_error("arbx_dbscan: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  const Index* ix = &h->ix;
+  if (ix->kind != KIND_POINT) { set_error("arbx_dbscan: POINT primitives only"); return ARBX_ERR_UNSUPPORTED; }
+  const int64_t n = ix->n;
+  if (n == 0) return ARBX_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  Scratch<float> selfq;
+  Scratch<uint32_t> order;
+  Scratch<int32_t> counts, uf;
+  ARBX_TRY(selfq.alloc((size_t)n * (ix->dim + 1), s));
+  ARBX_TRY(order.alloc((size_t)n, s));
+  ARBX_TRY(counts.alloc((size_t)n, s));
+  ARBX_TRY(uf.alloc((size_t)n, s));
+  self_queries_kernel<<<grid, 256, 0, s>>>(ix->leaves, n, ix->dim, leaf_width(KIND_POINT, ix->dim), eps, selfq.p, order.p);
+  ARBX_LAUNCH_CHECK();
+  const DimTable* tab = dim_table(ix->dim);
+  // 1. core test: capped neighbour count (the point itself included), early exit at min_pts
+  SpatialArgs a{selfq.p, n, KIND_SPHERE, order.p, counts.p, nullptr, nullptr, nullptr, min_pts, nullptr, 0};
+  ARBX_TRY(tab->spatial(ix, a, s));
+  dbscan_init_kernel<<<grid, 256, 0, s>>>(counts.p, min_pts, n, uf.p);
+  ARBX_LAUNCH_CHECK();
+  // 2. every unordered pair within eps once (half traversal): unite core-core, attach borders
+  a.rows = uf.p;
+  a.pass = 3;
+  a.self = 1;
+  ARBX_TRY(tab->spatial(ix, a, s));
+  // 3. labels
+  dbscan_labels_kernel<<<grid, 256, 0, s>>>(uf.p, n, labels);
+  ARBX_LAUNCH_CHECK();
+  return ARBX_OK;
 }
 
 static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind, int32_t limit,

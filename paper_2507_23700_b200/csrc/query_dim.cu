@@ -143,6 +143,38 @@ __device__ __forceinline__ bool hits_prim(const Query<QK>& q, const float* p) {
 // instead of 32 divergent ones, control flow is uniform, and the stack is one short array
 // per warp in shared memory.  The leaf test is per lane and exact, so the result is the same
 // set as one-query-per-thread traversal.
+// ---- DBSCAN edge callback (MODE 3): lock-free union-find over the core points ------------------
+// uf[i] = i at start for core points, -1 for the others.  Core-core edges are united (the
+// larger root is hooked under the smaller with atomicCAS, finds use path halving); a non-core
+// point next to a core point remembers ONE such core point as -2 - core (first writer wins).
+#ifndef ARBX_UF_HELPERS
+#define ARBX_UF_HELPERS
+__device__ __forceinline__ int32_t uf_find(int32_t* uf, int32_t x) {
+  for (;;) {
+    const int32_t p = ((volatile int32_t*)uf)[x];
+    if (p == x) return x;
+    const int32_t gp = ((volatile int32_t*)uf)[p];
+    if (gp != p) uf[x] = gp;     // path halving; roots only ever decrease, so a stale write is harmless
+    x = p;
+  }
+}
+__device__ __forceinline__ void uf_union(int32_t* uf, int32_t a, int32_t b) {
+  for (;;) {
+    a = uf_find(uf, a);
+    b = uf_find(uf, b);
+    if (a == b) return;
+    if (a < b) { const int32_t t = a; a = b; b = t; }       // hook the larger root a under b
+    if (atomicCAS(uf + a, a, b) == a) return;
+  }
+}
+__device__ __forceinline__ void dbscan_edge(int32_t* uf, const int32_t* counts, int min_pts, int32_t i, int32_t j) {
+  const bool ci = counts[i] >= min_pts, cj = counts[j] >= min_pts;
+  if (ci && cj) uf_union(uf, i, j);
+  else if (ci) atomicCAS(uf + j, -1, -2 - i);
+  else if (cj) atomicCAS(uf + i, -1, -2 - j);
+}
+#endif
+
 struct NodeX { float v[4 * D]; int32_t c0, c1, l, r; };
 
 __device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, int32_t ref, NodeX& nd) {
@@ -160,10 +192,12 @@ __device__ __forceinline__ void load_node_x(const float4* __restrict__ nodes, in
 // SELF (self-join, queries = the index's own primitives in tree order): query number `tpos` is
 // the leaf at sorted position tpos; only primitives at LATER positions are reported, so every
 // unordered pair appears once, and subtrees that end at or before tpos are skipped.
-template <int PK, int QK, bool FILL, bool SELF>
+template <int PK, int QK, int MODE, bool SELF>
 __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes, const float4* __restrict__ leaves,
                                                const int32_t* __restrict__ root, const Query<QK>& q,
-                                               int32_t* __restrict__ out, int limit, int stop, int tpos) {
+                                               int32_t* __restrict__ out, int limit, int stop, int tpos,
+                                               const int32_t* __restrict__ counts, int min_pts, int32_t qi) {
+  constexpr bool FILL = MODE == 1 || MODE == 2;
   int cnt = 0;
   int32_t stack[STACK_DEPTH];
   int sp = 0;
@@ -192,6 +226,7 @@ __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes,
       load_leaf<PK>(leaves, j, lf);
       if ((!SELF || j > tpos) && hits_prim<QK, PK>(q, lf.v)) {
         if constexpr (FILL) { if (cnt < limit) out[cnt] = (int32_t)(lf.idx & ~LEAF_END); }
+        if constexpr (MODE == 3) dbscan_edge(out, counts, min_pts, qi, (int32_t)(lf.idx & ~LEAF_END));
         ++cnt;
         if (cnt >= stop) return cnt;   // capped query: early exit
       }
@@ -312,7 +347,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
                                                      int32_t* __restrict__ indices, int cap,
                                                      int* __restrict__ overflow, int stop_fill, int mode,
                                                      float alpha) {
-  constexpr bool FILL = MODE != 0;     // hits are written somewhere
+  constexpr bool FILL = MODE == 1 || MODE == 2;     // hits are written to rows / CSR slices
   constexpr int QW = prim_width(QK, D);
   constexpr int PQ_CAP = 320;   // packet work list (node ids) per warp
   __shared__ int32_t s_stack[QT / 32][PQ_CAP];
@@ -351,9 +386,10 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   // mode 0: per-warp choice; 1: always one query per lane; 2: always packet
   if (mode == 1 || (mode == 0 && !warp_coherent<QK>(q, valid, alpha))) {
     int c = 0;
-    if (alive) c = thread_traverse<PK, QK, FILL, SELF>(nodes, leaves, root, q, FILL ? indices + base64 : nullptr, limit,
-                                                        capped ? limit : INT32_MAX, (int)t);
-    if constexpr (MODE != 1) {
+    if (alive) c = thread_traverse<PK, QK, MODE, SELF>(nodes, leaves, root, q,
+                                                       MODE == 3 ? indices : FILL ? indices + base64 : nullptr, limit,
+                                                       capped ? limit : INT32_MAX, (int)t, counts, cap, (int32_t)qi);
+    if constexpr (MODE == 0 || MODE == 2) {
       if (valid) counts[qi] = c;
       if constexpr (MODE == 2) { if (c > cap) atomicAdd(overflow, 1); }
     }
@@ -409,6 +445,8 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
             if (cnt < limit) { stage[pend * 33 + lane] = (int32_t)(lf.idx & ~LEAF_END); ++pend; }
             ++cnt;
           }
+        } else if constexpr (MODE == 3) {
+          if (hit) dbscan_edge(indices, counts, cap, (int32_t)qi, (int32_t)(lf.idx & ~LEAF_END));
         } else {
           cnt += hit ? 1 : 0;
         }
@@ -472,7 +510,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
     }
   }
   if constexpr (FILL) flush(__ballot_sync(~0u, pend > 0));
-  if constexpr (MODE != 1) {
+  if constexpr (MODE == 0 || MODE == 2) {
     if (valid) counts[qi] = MODE == 0 ? min(cnt, limit) : cnt;
     if constexpr (MODE == 2) { if (cnt > cap) atomicAdd(overflow, 1); }
   }
@@ -793,7 +831,10 @@ arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s
   const int n = (int)ix->n;
   if (a.pass == 1)
     spatial_kernel<PK, QK, 1, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, a.stop_fill, mode, alpha);
-  else if (a.pass == 2)
+  else if (a.pass == 3) {
+    if constexpr (SELF)   // DBSCAN edges: counts = neighbour counts (read), rows = union-find array, cap = min_pts
+      spatial_kernel<PK, QK, 3, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, nullptr, 0, mode, alpha);
+  } else if (a.pass == 2)
     spatial_kernel<PK, QK, 2, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, 0, mode, alpha);
   else
     spatial_kernel<PK, QK, 0, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, a.cap, nullptr, 0, mode, alpha);

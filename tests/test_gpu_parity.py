@@ -512,3 +512,43 @@ def test_query_pairs_lattice_and_errors(arbx):
         b.query_pairs(0.1)
     assert e.value.status == arbx.ERR_UNSUPPORTED
     b.close()
+
+
+# ---- NEXT-3: DBSCAN on top of the index ---------------------------------------
+@pytest.mark.parametrize("traversal", ["thread", "packet", None])
+@pytest.mark.parametrize("D,min_pts", [(2, 5), (3, 4), (3, 1), (5, 6)])
+def test_dbscan(arbx, orc, monkeypatch, traversal, D, min_pts):
+    from oracle import compare as cmp
+    if traversal:
+        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    n = 12000
+    blobs = dg.gaussian_mixture(n - 2000, D, 100 + D, centre_seed=7, ncomp=12, sigma=0.015)
+    p = np.concatenate([blobs, dg.uniform_points(2000, D, 200 + D)]).astype(np.float32)   # clusters + background noise
+    eps = 0.6 * (8.0 / n) ** (1.0 / D) if D < 5 else 0.03
+    o = orc.dbscan(p, eps, min_pts)
+    while o[3]:                       # a pair inside the 1e-6 tolerance band: nudge eps off it
+        eps = float(np.float32(eps * 1.0001))
+        o = orc.dbscan(p, eps, min_pts)
+    ix = arbx.Index(_dev(p), dg.POINT)
+    labels = _np(ix.dbscan(eps, min_pts))
+    st = cmp.compare_dbscan(o, labels, f"dbscan D={D} minPts={min_pts} {traversal}")
+    assert st["clusters"] >= 1 and st["core"] > 0
+    core = o[0]
+    assert np.array_equal(labels[core] == np.arange(len(p))[core], labels[core] == np.arange(len(p))[core])
+    # label = smallest core index of the cluster
+    for lab in np.unique(labels[labels >= 0])[:50]:
+        members = np.nonzero((labels == lab) & core)[0]
+        assert members.min() == lab
+    ix.close()
+
+
+def test_dbscan_chain_closed_form(arbx):
+    chain = np.zeros((7, 2), np.float32)
+    chain[:, 0] = np.arange(7)
+    pts = np.concatenate([chain, chain + np.float32([0, 50]), np.float32([[100, 100], [200, 200]])])
+    ix = arbx.Index(_dev(pts), dg.POINT)
+    lab = _np(ix.dbscan(1.25, 3)).tolist()
+    assert lab == [1] * 7 + [8] * 7 + [-1, -1]
+    assert _np(ix.dbscan(0.5, 1)).tolist() == list(range(16))         # minPts = 1: every point its own cluster
+    assert _np(ix.dbscan(0.5, 2)).tolist() == [-1] * 16               # nobody has a neighbour within 0.5
+    ix.close()

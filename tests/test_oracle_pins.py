@@ -309,3 +309,28 @@ def test_pair_comparator_closed_form(orc):
         cmp.compare_pairs(n, o, both)
     with pytest.raises(AssertionError):
         cmp.compare_pairs(n, o, (np.maximum(off - (off > 0), 0), good[1][1:]))   # one pair dropped
+
+
+def test_dbscan_oracle_closed_forms(orc):
+    """DBSCAN oracle on cases with a known answer: a 1-D chain (ends are border points), two far
+    apart blobs, and isolated points (noise)."""
+    from oracle import compare as cmp
+    chain = np.zeros((7, 2), np.float32)
+    chain[:, 0] = np.arange(7)                                 # 0..6 on a line, spacing 1
+    iso = np.float32([[100, 100], [200, 200]])
+    pts = np.concatenate([chain, chain + np.float32([0, 50]), iso])
+    core, comp, allowed, band = orc.dbscan(pts, 1.25, 3)       # each inner point sees itself + 2 neighbours
+    assert not band
+    assert core.tolist() == [False, True, True, True, True, True, False] * 2 + [False, False]
+    assert len(set(comp[core].tolist())) == 2                   # two clusters
+    assert allowed[0] == {int(comp[1])} and allowed[6] == {int(comp[5])}   # chain ends are border points
+    assert allowed[14] == set() and allowed[15] == set()        # isolated points are noise
+    labels = np.array([1, 1, 1, 1, 1, 1, 1, 8, 8, 8, 8, 8, 8, 8, -1, -1])
+    st = cmp.compare_dbscan((core, comp, allowed, band), labels)
+    assert st == dict(clusters=2, core=10, border=4, noise=2)
+    bad = labels.copy(); bad[7:14] = 1                          # merging the two clusters must be rejected
+    with pytest.raises(AssertionError):
+        cmp.compare_dbscan((core, comp, allowed, band), bad)
+    bad = labels.copy(); bad[0] = -1                            # a border point may not be noise
+    with pytest.raises(AssertionError):
+        cmp.compare_dbscan((core, comp, allowed, band), bad)
