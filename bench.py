@@ -137,47 +137,79 @@ def rank_seed_offset(rank: int) -> int:
 
 
 class ClockSampler:
-    """nvidia-smi clocks/throttle reasons DURING the timed region (B200_PROFILING.md)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons DURING the timed region (B200_PROFILING.md).
+    Sampling from another thread or process (a looping `nvidia-smi --query-gpu`, or NVML polled
+    from a thread) was measured to stall this process's CUDA calls by 2-60 ms per step: NVML
+    queries and the CUDA allocator contend for a driver lock.  So the samples are taken through
+    NVML by the BENCH THREAD ITSELF, once per step, right after the step's last kernel has been
+    enqueued: the GPU is busy with that kernel (milliseconds of queued work) while the host
+    asks.  Without pynvml the fallback is a looping nvidia-smi at 200 ms."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
     def __init__(self, index: int):
-        self.rows = []
+        self.rows = []          # (time, sm_mhz, reasons bitmask)
+        self.smax = None
         self.proc = None
+        self.nv = None
         try:
-            self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
-                 "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.smax = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.nv = pynvml
         except Exception:
-            self.proc = None
+            try:
+                q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                     "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+                self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "200",
+                                              "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                threading.Thread(target=self._read, daemon=True).start()
+            except Exception:
+                self.proc = None
+
+    def sample(self):
+        """One in-thread NVML sample (call while the GPU has queued work)."""
+        if self.nv is None:
+            return
+        try:
+            mhz = float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+            try:
+                bits = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+            except Exception:
+                bits = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            self.rows.append((time.time(), mhz, bits))
+        except Exception:
+            pass
 
     def _read(self):
+        names = [0x8, 0x40, 0x20, 0x4]
         for line in self.proc.stdout:
-            self.rows.append((time.time(), line.strip()))
-
-    def stop(self, t0: float, t1: float) -> dict:
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        sm, smax, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.2] or [r for (_, r) in self.rows]
-        for r in rows:
-            f = [x.strip() for x in r.split(",")]
+            f = [x.strip() for x in line.split(",")]
             try:
-                sm.append(float(f[0])); smax.append(float(f[1]))
+                bits = 0
+                for nm, v in zip(names, f[2:6]):
+                    if v.lower().startswith("active"):
+                        bits |= nm
+                self.smax = float(f[1])
+                self.rows.append((time.time(), float(f[0]), bits))
             except Exception:
                 continue
-            for nm, v in zip(names, f[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(nm)
-        return {"sm_mhz": float(np.median(sm)) if sm else None,
-                "sm_max_mhz": float(max(smax)) if smax else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is not None:
+            time.sleep(0.25)
+            self.proc.terminate()
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": self.smax, "reasons": ["clock sampling unavailable"], "samples": 0}
+        rows = [r for r in self.rows if t0 <= r[0] <= t1 + 0.1] or self.rows
+        bits = 0
+        for r in rows:
+            bits |= r[2]
+        return {"sm_mhz": float(np.median([r[1] for r in rows])), "sm_max_mhz": self.smax,
+                "reasons": sorted(v for k, v in self.REASONS.items() if bits & k), "samples": len(rows),
+                "source": "nvml, one sample per step while the step's last kernel runs" if self.nv is not None else "nvidia-smi -lms 200"}
 
 
 # ---- the oracle, timed (cpu_baseline leg and --impl reference) ----------------------------------
@@ -311,6 +343,7 @@ def main():
     nbatches = 3 if k else 2
 
     marks = []   # (name, event) per step, on `stream`
+    sampler_box = [None]
 
     def mark(name):
         e = torch.cuda.Event(enable_timing=True)
@@ -327,6 +360,8 @@ def main():
         if k:
             arbx.arbx_query_knn(h, qpoints, nq, k, kidx, kdist, stream)
             if timed_marks: mark("knn")
+        if timed_marks and sampler_box[0] is not None:
+            sampler_box[0].sample()      # the GPU is busy with the kernels just enqueued
         arbx.arbx_destroy(h, stream)
 
     # ---- value leg: inputs resident in HBM --------------------------------------------------------
@@ -334,7 +369,8 @@ def main():
         for _ in range(args.warmup):
             step(d_prims, d_queries, d_qpoints, False)
         barrier()
-        sampler = ClockSampler(local_rank) if rank == 0 else None
+        sampler = ClockSampler(local_rank) if rank == 0 and not os.environ.get("ARBX_BENCH_NO_SMI") else None
+        sampler_box[0] = sampler
         arbx.arbx_profile_enable(True)
         arbx.arbx_profile_read()
         l0 = arbx.arbx_launch_count()
@@ -350,6 +386,7 @@ def main():
         launches = arbx.arbx_launch_count() - l0
         prof = arbx.arbx_profile_read()
         arbx.arbx_profile_enable(False)
+        sampler_box[0] = None
         clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     ms_total = e0.elapsed_time(e1)
     calls = {}
