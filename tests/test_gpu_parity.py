@@ -552,3 +552,26 @@ def test_dbscan_chain_closed_form(arbx):
     assert _np(ix.dbscan(0.5, 1)).tolist() == list(range(16))         # minPts = 1: every point its own cluster
     assert _np(ix.dbscan(0.5, 2)).tolist() == [-1] * 16               # nobody has a neighbour within 0.5
     ix.close()
+
+
+def test_self_join_and_dbscan_tiny_and_1d(arbx, orc):
+    from oracle import compare as cmp
+    for n in (1, 2, 3, 17):
+        p = dg.uniform_points(n, 1, 300 + n)
+        ix = arbx.Index(_dev(p).reshape(n, 1), dg.POINT, dim=1)
+        off, idx = ix.query_pairs(10.0)                       # everything within reach: all n(n-1)/2 pairs
+        assert idx.numel() == n * (n - 1) // 2 and _np(off)[-1] == idx.numel()
+        lab = _np(ix.dbscan(10.0, 1))
+        assert np.all(lab == 0)                               # one cluster, named after its smallest core index
+        assert np.all(_np(ix.dbscan(10.0, n + 1)) == -1)      # nobody reaches minPts
+        ix.close()
+    x = np.sort(dg.uniform_points(4000, 1, 311), axis=0)
+    ix = arbx.Index(_dev(x), dg.POINT)
+    r = 0.0007
+    o = orc.spatial(x, dg.POINT, dg.sphere_queries(x, r), dg.SPHERE)
+    off, idx = ix.query_pairs(r)
+    cmp.compare_pairs(len(x), o, (_np(off), _np(idx)), "pairs 1-D")
+    od = orc.dbscan(x, r, 3)
+    if not od[3]:
+        cmp.compare_dbscan(od, _np(ix.dbscan(r, 3)), "dbscan 1-D")
+    ix.close()
