@@ -3,8 +3,13 @@
 // PAPER.md:L69 (radius / nearest predicates), L79 (nearest = distance to the stored geometry),
 // L104-115 (callback / storage queries), L295 + L307 (traversal, sorted queries), L303 (count).
 //
-// One query per thread; the 32 queries of a warp are neighbours on the space-filling curve
-// (qorder), so they walk nearly the same nodes and the node fetches hit L1/L2.
+// Also the traversal forms of the NEXT items: capped count / capped fill (early exit), the
+// self-join (SELF: half traversal over the index's own leaves) and the DBSCAN edge callback
+// (MODE 3).
+//
+// The 32 queries of a warp are neighbours on the space-filling curve (qorder).  Spatial
+// queries pick, per warp, a warp-cooperative packet traversal (coherent queries) or one
+// independent traversal per lane; kNN runs one traversal per lane.
 #include <algorithm>
 #include <cstdlib>
 #include <cstdint>
@@ -736,7 +741,7 @@ __global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ node
 // ---- one query per thread (independent traversal) --------------------------------------------------
 // Kept beside the packet kernels: when the 32 queries of a warp are NOT spatially coherent
 // (high dimension, strongly clustered data) the packet visits the union of 32 unrelated
-// paths and independent traversal wins.  The host picks per call (see pick_packet below).
+// paths and independent traversal wins.  Spatial kernels choose per warp (warp_coherent).
 template <int PK, class Heap>
 __global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict__ nodes,
                                                  const float4* __restrict__ leaves,
