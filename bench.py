@@ -17,7 +17,9 @@ metric is quoted on ("... at N=10M fp32 3D").
 value       = queries answered per second over the whole step (3 query batches; the build
               is inside the step), inputs resident in HBM, device-timed.
 e2e         = the same with pinned-HOST inputs copied to the device and every result copied
-              back to pinned host memory inside the timed region.
+              back to pinned host memory inside the timed region, every step; three streams
+              and two buffer sets let step i's compute overlap step i+1's copy-in and step
+              i-1's copy-out (the per-call stream argument of the ABI).
 breakdown   = per-call rates: build Mprims/s, radius/count/kNN queries/s, and per hot-path
               step milliseconds + achieved algorithmic GB/s (arbx_profile_*, CUDA events).
 roofline    = the dominant kernel (largest share of the step) against the measured HBM peak.
@@ -354,15 +356,16 @@ def main():
         e.record(stream)
         marks.append((name, e))
 
-    def step(prims, queries, qpoints, timed_marks):
+    def step(prims, queries, qpoints, timed_marks, out=None):
+        o_off, o_idx, o_cnt, o_ki, o_kd = out if out is not None else (offsets, indices, counts, kidx, kdist)
         h = arbx.arbx_build(prims, D, pk, stream)
         if timed_marks: mark("build")
-        arbx.arbx_query_spatial(h, queries, nq, qk, offsets, indices, capacity, stream)
+        arbx.arbx_query_spatial(h, queries, nq, qk, o_off, o_idx, capacity, stream)
         if timed_marks: mark("spatial")
-        arbx.arbx_query_count(h, queries, nq, qk, counts, stream)
+        arbx.arbx_query_count(h, queries, nq, qk, o_cnt, stream)
         if timed_marks: mark("count")
         if k:
-            arbx.arbx_query_knn(h, qpoints, nq, k, kidx, kdist, stream)
+            arbx.arbx_query_knn(h, qpoints, nq, k, o_ki, o_kd, stream)
             if timed_marks: mark("knn")
         if timed_marks and sampler_box[0] is not None and step_no[0] in sample_steps:
             sampler_box[0].sample()      # the GPU is busy with the kernels just enqueued
@@ -449,30 +452,61 @@ def main():
         hc = torch.empty(nq, dtype=torch.int32).pin_memory()
         hki = torch.empty((nq, k), dtype=torch.int32).pin_memory() if k else None
         hkd = torch.empty((nq, k), dtype=torch.float32).pin_memory() if k else None
-        s_prims, s_queries = torch.empty_like(d_prims), torch.empty_like(d_queries)
-        s_qpoints = torch.empty_like(d_qpoints) if k else None
+        # Three streams, double-buffered: while step i computes, the inputs of step i+1 are coming
+        # in and the results of step i-1 are going out (H2D and D2H use separate copy engines).
+        # Every step still copies all of its inputs in and all of its results out.
+        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+        inb = [(torch.empty_like(d_prims), torch.empty_like(d_queries), torch.empty_like(d_qpoints) if k else None)
+               for _ in range(2)]
+        outb = [(offsets, indices, counts, kidx, kdist),
+                (torch.empty_like(offsets), torch.empty_like(indices), torch.empty_like(counts),
+                 torch.empty_like(kidx) if k else None, torch.empty_like(kdist) if k else None)]
+        ev_in, ev_comp, ev_out = [None, None], [None, None], [None, None]
 
-        def e2e_step():
-            s_prims.copy_(h_prims, non_blocking=True)
-            s_queries.copy_(h_queries, non_blocking=True)
-            if k: s_qpoints.copy_(h_qpoints, non_blocking=True)
-            step(s_prims, s_queries, s_qpoints, False)
-            ho.copy_(offsets, non_blocking=True)
-            hi[:capacity].copy_(indices[:capacity], non_blocking=True)
-            hc.copy_(counts, non_blocking=True)
-            if k:
-                hki.copy_(kidx, non_blocking=True)
-                hkd.copy_(kdist, non_blocking=True)
+        def enqueue_in(i):
+            b = i % 2
+            with torch.cuda.stream(s_in):
+                if ev_comp[b] is not None: s_in.wait_event(ev_comp[b])     # step i-2 is done with this buffer
+                inb[b][0].copy_(h_prims, non_blocking=True)
+                inb[b][1].copy_(h_queries, non_blocking=True)
+                if k: inb[b][2].copy_(h_qpoints, non_blocking=True)
+                ev_in[b] = torch.cuda.Event(); ev_in[b].record(s_in)
 
-        with torch.cuda.stream(stream):
-            e2e_step()
-            barrier()
-            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            for _ in range(args.steps):
-                e2e_step()
-            b.record(stream)
-            barrier()
+        def run(i):
+            b = i % 2
+            stream.wait_event(ev_in[b])
+            if ev_out[b] is not None: stream.wait_event(ev_out[b])          # results of step i-2 have left
+            with torch.cuda.stream(stream):
+                step(inb[b][0], inb[b][1], inb[b][2], False, outb[b])
+            ev_comp[b] = torch.cuda.Event(); ev_comp[b].record(stream)
+
+        def enqueue_out(i):
+            b = i % 2
+            o_off, o_idx, o_cnt, o_ki, o_kd = outb[b]
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(ev_comp[b])
+                ho.copy_(o_off, non_blocking=True)
+                hi[:capacity].copy_(o_idx[:capacity], non_blocking=True)
+                hc.copy_(o_cnt, non_blocking=True)
+                if k:
+                    hki.copy_(o_ki, non_blocking=True)
+                    hkd.copy_(o_kd, non_blocking=True)
+                ev_out[b] = torch.cuda.Event(); ev_out[b].record(s_out)
+
+        def pipeline(nsteps):
+            enqueue_in(0)
+            for i in range(nsteps):
+                if i + 1 < nsteps: enqueue_in(i + 1)
+                run(i)
+                enqueue_out(i)
+
+        pipeline(2)                       # warm-up (allocator, second buffer set)
+        barrier()
+        a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+        a.record(s_in)
+        pipeline(args.steps)
+        b.record(s_out)
+        barrier()
         ms_e2e = a.elapsed_time(b) / args.steps
         h2d = h_prims.numel() * 4 + h_queries.numel() * 4 + (h_qpoints.numel() * 4 if k else 0)
         d2h = ho.numel() * 4 + capacity * 4 + hc.numel() * 4 + (hki.numel() * 8 if k else 0)
