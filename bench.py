@@ -404,6 +404,11 @@ def main():
         if nb_ != "begin":
             calls[nb_] = calls.get(nb_, 0.0) + ea.elapsed_time(eb)
     calls = {c: v / args.steps for c, v in calls.items()}
+    # per-step durations (begin of step i -> begin of step i+1; the last one ends at e1): a host
+    # hiccup (the storage query synchronises once per call) shows up as max >> median
+    begins = [e for (nm, e) in marks if nm == "begin"]
+    per_step = [a.elapsed_time(b) for a, b in zip(begins[:-1], begins[1:])] + [begins[-1].elapsed_time(e1)]
+    step_stats = dict(min=round(min(per_step), 4), median=round(float(np.median(per_step)), 4), max=round(max(per_step), 4))
     marks.clear()
 
     # ---- outside the step: the capped count (NEXT-1, arbx_query_count_upto), device-timed ---------------
@@ -546,7 +551,7 @@ def main():
             radius_csr_qps=round(nq / calls["spatial"] * 1e3, 1), radius_csr_ms=round(calls["spatial"], 4),
             count_only_qps=round(nq / calls["count"] * 1e3, 1), count_only_ms=round(calls["count"], 4),
             knn_qps=round(nq / calls["knn"] * 1e3, 1) if k else None, knn_ms=round(calls["knn"], 4) if k else None,
-            pairs=capacity, extras_outside_step=extras, kernels=kern)
+            pairs=capacity, step_ms=step_stats, extras_outside_step=extras, kernels=kern)
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             import oracle
