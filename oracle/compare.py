@@ -65,11 +65,22 @@ def compare_counts(orc, counts, what: str = "") -> None:
     assert not bad.any(), f"{what}: {int(bad.sum())} counts outside [sure, sure+band], first q={int(np.argmax(bad))}"
 
 
-def compare_knn(prims, pkind: int, qpoints, k: int, orc, got, eps: float = EPS, what: str = "",
-                abs_tol: float = 0.0) -> None:
+def _sphere_slack(prims, dim: int, idx, d) -> np.ndarray:
+    """Per-pair absolute slack for SPHERE primitives, where the fp32 distance ||y-c|| - R
+    cancels: |error| <= 4 * 2^-23 * (||y-c|| + R) <= 2^-21 * (d + 2R), because
+    ||y-c|| <= d + R.  idx < 0 (padding) gets 0."""
+    idx = np.asarray(idx)
+    R = np.where(idx >= 0, prims[np.maximum(idx, 0), dim].astype(np.float64), 0.0)
+    dd = np.where(np.isfinite(d), d, 0.0)
+    return 2.0 ** -21 * (dd + 2.0 * R)
+
+
+def compare_knn(prims, pkind: int, qpoints, k: int, orc, got, eps: float = EPS, what: str = "") -> None:
     """orc = (idx[nq,k], dist64[nq,k]); got = (idx[nq,k] int32, dist[nq,k] fp32 or None).
-    abs_tol: absolute slack added to every distance tolerance (sphere primitives only, where
-    ||y-c|| - R cancels)."""
+    For SPHERE primitives every distance tolerance is widened by the per-pair cancellation
+    bound of _sphere_slack (position-wise rules use the largest slack of the row, since fp32
+    keys that differ by less than the slack may swap places)."""
+    SPHERE = 2
     o_idx, o_d = orc
     g_idx, g_d = got
     g_idx = np.asarray(g_idx)
@@ -88,6 +99,12 @@ def compare_knn(prims, pkind: int, qpoints, k: int, orc, got, eps: float = EPS, 
     qids = np.repeat(np.arange(nq, dtype=np.int64), kk)
     d_true = knn_distance_pairs(prims, pkind, qpoints, qids, g_idx[:, :kk].reshape(-1)).reshape(nq, kk)
     Dk = o_d[:, kk - 1][:, None]
+    if pkind == SPHERE:
+        dim = qpoints.shape[1]
+        pair_tol = _sphere_slack(prims, dim, g_idx[:, :kk], d_true)
+        abs_tol = np.maximum(pair_tol, _sphere_slack(prims, dim, o_idx[:, :kk], o_d[:, :kk])).max(axis=1)[:, None]
+    else:
+        pair_tol = abs_tol = 0.0
     # (5b) every reported neighbour lies within D_k(1+eps)
     assert np.all(d_true <= Dk * (1 + eps) + abs_tol), f"{what}: reported neighbour farther than D_k(1+eps)"
     # (5a) every oracle neighbour strictly closer than D_k(1-eps) is reported
@@ -106,7 +123,7 @@ def compare_knn(prims, pkind: int, qpoints, k: int, orc, got, eps: float = EPS, 
         assert np.all(np.abs(gd - od) <= eps * od + abs_tol), (
             f"{what}: distance mismatch, max rel {np.max(np.abs(gd - od) / np.maximum(od, 1e-300)):.3e}")
         # (4) the reported distance belongs to the reported index
-        assert np.all(np.abs(gd - d_true) <= eps * d_true + abs_tol), f"{what}: distance does not match its index"
+        assert np.all(np.abs(gd - d_true) <= eps * d_true + pair_tol), f"{what}: distance does not match its index"
 
 
 def compare_counts_upto(orc, counts, limit: int, what: str = "") -> None:

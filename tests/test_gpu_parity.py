@@ -108,8 +108,7 @@ def test_all_cells_small(arbx, orc, D, pkind):
         gi, gd = ix.query_knn(_dev(qp), k)
         ix.close()
         o = orc.knn(prims, pkind, qp, k)
-        tol = 4e-6 * float(np.abs(prims).max()) if pkind == dg.SPHERE else 0.0
-        cmp.compare_knn(prims, pkind, qp, k, o, (_np(gi), _np(gd)), what=f"knn D={D} pk={pkind} k={k}", abs_tol=tol)
+        cmp.compare_knn(prims, pkind, qp, k, o, (_np(gi), _np(gd)), what=f"knn D={D} pk={pkind} k={k}")
 
 
 @pytest.mark.parametrize("leaf_max", [1, 2, 8, 64])

@@ -334,3 +334,204 @@ def test_dbscan_oracle_closed_forms(orc):
     bad = labels.copy(); bad[0] = -1                            # a border point may not be noise
     with pytest.raises(AssertionError):
         cmp.compare_dbscan((core, comp, allowed, band), bad)
+
+
+# ---- hand-worked cases for every cell of the predicate table ---------------------------------------
+CELLS = os.path.join(os.path.dirname(__file__), "golden", "predicate_cells.txt")
+_KIND = {"P": dg.POINT, "B": dg.BOX, "S": dg.SPHERE}
+_ARITH = {("S", "P"), ("S", "B"), ("S", "S"), ("B", "S"), ("P", "S")}   # predicates with arithmetic (a band exists)
+
+
+def _cell_cases():
+    out = []
+    for ln, line in enumerate(open(CELLS), 1):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        head, q, p, expect = [t.strip() for t in line.split("|")]
+        qk, pk, D = head.split()
+        out.append(pytest.param(qk, pk, int(D), np.float32(q.split()), np.float32(p.split()), expect,
+                                id=f"L{ln}-{qk}x{pk}-D{D}-{expect}"))
+    return out
+
+
+@pytest.mark.parametrize("qk,pk,D,q,p,expect", _cell_cases())
+def test_predicate_cells_hand_worked(orc, qk, pk, D, q, p, expect):
+    """tests/golden/predicate_cells.txt: one hit, one miss and one exactly-touching pair (and the
+    mirrored / single-axis variants) for every (query kind x primitive kind) cell, D in {1,3}.
+    Checked in brute force and through the grid (alone and among far-away decoys)."""
+    width = {"P": D, "B": 2 * D, "S": D + 1}
+    assert len(q) == width[qk] and len(p) == width[pk]
+    decoys = np.tile(p, (5, 1))
+    decoys[:, :D] += np.float32(1000.0) * np.arange(1, 6, dtype=np.float32)[:, None]   # far away on every axis
+    if pk == "B":
+        decoys[:, D:] += np.float32(1000.0) * np.arange(1, 6, dtype=np.float32)[:, None]
+    many = np.concatenate([decoys[:2], p[None, :], decoys[2:]])
+    for prims, at in ((p[None, :], 0), (many, 2)):
+        for grid in [None, orc.Grid(prims, _KIND[pk], 1.0), orc.Grid(prims, _KIND[pk], 0.3)]:
+            off, idx, band = orc.spatial(prims, _KIND[pk], q[None, :], _KIND[qk], grid)
+            if expect == "miss":
+                assert int(off[-1]) == 0, "a miss was reported"
+                continue
+            assert idx.tolist() == [at], "the match is missing"
+            T_is_zero = (qk == "S" and pk != "S" and q[D] == 0) or (pk == "S" and qk != "S" and p[D] == 0)
+            want_band = expect == "touch" and (qk, pk) in _ARITH and not T_is_zero
+            assert bool(band[0]) == want_band, "boundary pair must be flagged iff the predicate has arithmetic"
+
+
+@pytest.mark.parametrize("D", [1, 2, 3])
+def test_unit_cells_queried_by_half_radius_sphere(orc, D):
+    """SPHERE query x BOX primitives on the unit-cell lattice: a ball of radius 1/2 at a cell
+    centre holds the cell itself (distance 0) and touches its 2D face neighbours at exactly
+    1/2; edge neighbours are at sqrt(2)/2 > 1/2."""
+    g = 5
+    cells = dg.lattice_cells(g, D)
+    q = np.float32([[2.5] * D + [0.5]])
+    for grid in _modes(orc, cells, dg.BOX, "spatial", 0.5):
+        off, idx, band = orc.spatial(cells, dg.BOX, q, dg.SPHERE, grid)
+        assert int(off[-1]) == 1 + 2 * D and int(band.sum()) == 2 * D
+        own = idx[band == 0]
+        assert len(own) == 1 and np.array_equal(cells[own[0], :D], np.full(D, 2.0, np.float32))
+        l1 = np.abs(cells[idx[band == 1], :D] - 2.0).sum(1)
+        assert np.all(l1 == 1.0)
+    # radius 3/4: a neighbour cell offset on j axes is at distance sqrt(j)/2 -> the 2D face cells
+    # (0.5) and the 2D(D-1) edge cells (0.707) are inside, the corner cells (0.866) are not
+    q2 = np.float32([[2.5] * D + [0.75]])
+    off, idx, band = orc.spatial(cells, dg.BOX, q2, dg.SPHERE)
+    expect = 1 + 2 * D + (2 * D * (D - 1) if D >= 2 else 0)
+    assert int(off[-1]) == expect and not band.any()
+
+
+# ---- the comparators reject wrong answers --------------------------------------------------------------
+def _small_spatial(orc):
+    p = dg.uniform_points(400, 3, 1)
+    q = dg.sphere_queries(dg.uniform_points(60, 3, 2), 0.2)
+    o = orc.spatial(p, dg.POINT, q, dg.SPHERE)
+    assert not o[2].any() and int(o[0][-1]) > 200
+    return p, q, o
+
+
+def test_compare_spatial_and_counts_reject_corruption(orc):
+    from oracle import compare as cmp
+    p, q, o = _small_spatial(orc)
+    n = len(p)
+    off, idx = o[0].copy(), o[1].copy()
+    cmp.compare_spatial(n, o, (off, idx))                          # the oracle's own answer passes
+    cmp.compare_counts(o, np.diff(off))
+    g = dg.rng(5)
+    shuffled = idx.copy()
+    for j in range(len(off) - 1):                                  # order inside a row is free
+        shuffled[off[j]:off[j + 1]] = g.permutation(shuffled[off[j]:off[j + 1]])
+    cmp.compare_spatial(n, o, (off, shuffled))
+    row = int(np.argmax(np.diff(off) >= 2))
+    # a dropped pair
+    o2 = off.copy(); o2[row + 1:] -= 1
+    with pytest.raises(AssertionError, match="missing"):
+        cmp.compare_spatial(n, o, (o2, np.delete(idx, off[row])))
+    # a foreign index (a primitive that does not match) in place of a real one
+    foreign = np.setdiff1d(np.arange(n), idx[off[row]:off[row + 1]])[0]
+    bad = idx.copy(); bad[off[row]] = foreign
+    with pytest.raises(AssertionError):
+        cmp.compare_spatial(n, o, (off, bad))
+    # an extra pair
+    o3 = off.copy(); o3[row + 1:] += 1
+    with pytest.raises(AssertionError, match="neither sure nor band"):
+        cmp.compare_spatial(n, o, (o3, np.insert(idx, off[row], foreign)))
+    # a duplicated index inside a row
+    dup = idx.copy(); dup[off[row]] = dup[off[row] + 1]
+    with pytest.raises(AssertionError):
+        cmp.compare_spatial(n, o, (off, dup))
+    # an index out of range, offsets that do not start at 0 / decrease / disagree with len(indices)
+    oob = idx.copy(); oob[0] = n
+    with pytest.raises(AssertionError):
+        cmp.compare_spatial(n, o, (off, oob))
+    with pytest.raises(AssertionError):
+        cmp.compare_spatial(n, o, (off + 1, idx))
+    with pytest.raises(AssertionError):
+        cmp.compare_spatial(n, o, (off, idx[:-1]))
+    # counts off by one in either direction
+    for delta in (+1, -1):
+        c = np.diff(off).copy(); c[row] += delta
+        with pytest.raises(AssertionError, match="counts outside"):
+            cmp.compare_counts(o, c)
+
+
+def test_compare_spatial_band_pairs_are_optional_but_nothing_else(orc):
+    from oracle import compare as cmp
+    p = dg.lattice_points(4, 3)
+    q = dg.sphere_queries(p, 1.0)                                  # axis neighbours sit exactly at d = r: band
+    o = orc.spatial(p, dg.POINT, q, dg.SPHERE)
+    n = len(p)
+    assert o[2].sum() == 2 * 3 * 16 * 3 and (o[2] == 0).sum() == n
+    cmp.compare_spatial(n, o, (o[0], o[1]))                        # with every band pair
+    only_self = (np.arange(n + 1, dtype=np.int64), np.arange(n, dtype=np.int32))
+    cmp.compare_spatial(n, o, only_self)                           # with none of them
+    cmp.compare_counts(o, np.ones(n, dtype=np.int64))
+    with pytest.raises(AssertionError):
+        cmp.compare_counts(o, np.zeros(n, dtype=np.int64))         # the sure (self) pair is not optional
+    with pytest.raises(AssertionError):
+        cmp.compare_counts(o, np.diff(o[0]) + 1)
+
+
+def test_compare_knn_rejects_corruption(orc):
+    from oracle import compare as cmp
+    p = dg.uniform_points(500, 3, 3)
+    qp = dg.uniform_points(40, 3, 4)
+    k = 6
+    o = orc.knn(p, dg.POINT, qp, k)
+    gi, gd = o[0].copy(), o[1].astype(np.float32)
+    cmp.compare_knn(p, dg.POINT, qp, k, o, (gi, gd))               # fp32-rounded oracle answer passes
+    cmp.compare_knn(p, dg.POINT, qp, k, o, (gi, None))             # distances are optional
+    # a distance off by 5e-6 relative
+    bad = gd.copy(); bad[3, 2] = np.float32(bad[3, 2] * (1 + 5e-6))
+    with pytest.raises(AssertionError):
+        cmp.compare_knn(p, dg.POINT, qp, k, o, (gi, bad))
+    # a wrong neighbour (a far primitive) with the right distance column
+    far = int(np.argmax(((p - qp[5]) ** 2).sum(1)))
+    wi = gi.copy(); wi[5, k - 1] = far
+    with pytest.raises(AssertionError):
+        cmp.compare_knn(p, dg.POINT, qp, k, o, (wi, gd))
+    with pytest.raises(AssertionError):
+        cmp.compare_knn(p, dg.POINT, qp, k, o, (wi, None))
+    # a duplicate neighbour
+    di = gi.copy(); di[7, 1] = di[7, 0]
+    with pytest.raises(AssertionError, match="duplicate"):
+        cmp.compare_knn(p, dg.POINT, qp, k, o, (di, gd))
+    # the (k+1)-th neighbour in place of the k-th (clearly farther than D_k)
+    o7 = orc.knn(p, dg.POINT, qp, k + 1)
+    assert np.all(o7[1][:, k] > o7[1][:, k - 1] * (1 + 1e-5))
+    si = gi.copy(); si[:, k - 1] = o7[0][:, k]
+    sd = gd.copy(); sd[:, k - 1] = o7[1][:, k]
+    with pytest.raises(AssertionError):
+        cmp.compare_knn(p, dg.POINT, qp, k, o, (si, sd))
+    # descending rows, an invalid index, padding where none is due
+    with pytest.raises(AssertionError):
+        cmp.compare_knn(p, dg.POINT, qp, k, o, (gi[:, ::-1].copy(), gd[:, ::-1].copy()))
+    ii = gi.copy(); ii[0, 0] = -1
+    with pytest.raises(AssertionError):
+        cmp.compare_knn(p, dg.POINT, qp, k, o, (ii, gd))
+    # n < k: padding is required
+    o3 = orc.knn(p[:4], dg.POINT, qp, k)
+    cmp.compare_knn(p[:4], dg.POINT, qp, k, o3, (o3[0], o3[1].astype(np.float32)))
+    np_ = o3[0].copy(); np_[:, 4:] = 0
+    with pytest.raises(AssertionError, match="padding"):
+        cmp.compare_knn(p[:4], dg.POINT, qp, k, o3, (np_, o3[1].astype(np.float32)))
+
+
+def test_compare_knn_sphere_tolerance_is_per_pair(orc):
+    """Sphere primitives: fp32 ||y-c|| - R cancels, so compare_knn widens the tolerance by the
+    per-pair bound 2^-21 (d + 2R) and by nothing more."""
+    from oracle import compare as cmp
+    s = np.float32([[0, 0, 0, 1000.0], [3000, 0, 0, 1.0], [0, 5000, 0, 2.0]])
+    y = np.float32([[1000.5, 0, 0]])                               # 0.5 outside a sphere of radius 1000
+    o = orc.knn(s, dg.SPHERE, y, 3)
+    assert o[0][0].tolist() == [0, 1, 2] and o[1][0, 0] == 0.5
+    gd = o[1].astype(np.float32)
+    ok = gd.copy(); ok[0, 0] = np.float32(0.5 + 2.0 ** -21 * 2000.0)       # inside the cancellation bound
+    cmp.compare_knn(s, dg.SPHERE, y, 3, o, (o[0], ok))
+    bad = gd.copy(); bad[0, 0] = np.float32(0.5 + 2.0 ** -21 * 2100.0 + 1e-6)
+    with pytest.raises(AssertionError):
+        cmp.compare_knn(s, dg.SPHERE, y, 3, o, (o[0], bad))
+    bad2 = gd.copy(); bad2[0, 1] = np.float32(bad2[0, 1] * (1 + 4e-6))      # 4e-6 relative is far outside eps + slack
+    with pytest.raises(AssertionError):
+        cmp.compare_knn(s, dg.SPHERE, y, 3, o, (o[0], bad2))
