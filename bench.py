@@ -56,20 +56,37 @@ def _peaks():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-# ---- algorithmic HBM bytes per hot-path step ----------
+# ---- algorithmic HBM bytes per hot-path step -------------
+def sort_passes(n, D):
+    """8-bit digit passes of the build sort: code width adapted to n (csrc/build.cu, reading A15)."""
+    lg = max(0, int(n - 1).bit_length())
+    b = (lg + D - 1) // D + 4
+    passes = (D * b + 7) // 8
+    b = min(min(32, 64 // D), max(b, 8 * passes // D))
+    return (D * b + 7) // 8
+
+
 def algorithmic_bytes(cfg, totals):
-    """Bytes the method itself must move per step, per kernel id of arbx_profile_kernel_name."""
+    """COMPULSORY bytes the method itself must move per step, per kernel id of
+    arbx_profile_kernel_name: SURVEY.md §8(d)'s per-primitive / per-query figures times the
+    units one step processes.  A traversal reads the part of the tree its queries can reach
+    ONCE: (leaf record + one child box + 8 bytes of links) per TOUCHED primitive, where
+    `touched` = distinct primitives that appear in this workload's results (measured, passed
+    in `totals`); `whole_tree` (every leaf and every node slot) is reported beside it."""
     n, nq, D = cfg["n"], cfg["nq"], cfg["dim"]
     pk, qk = cfg["pkind"], cfg["qkind"]
     pw = D if pk == 0 else 2 * D if pk == 1 else D + 1          # floats per primitive row
     qw = D if qk == 0 else 2 * D if qk == 1 else D + 1          # floats per spatial query row
-    lw = (pw + 1 + 3) // 4 * 4                                  # floats per leaf record
-    nw = 4 * (D + 1)                                            # floats per internal node
-    npass = (D * min(32, 64 // D) + 7) // 8                     # 8-bit digit passes, build sort
+    lw = (pw + 1 + 1) // 2 * 2                                  # floats per leaf record as SURVEY.md counts it
+                                                                # (geometry + index, 8-byte granules: 16 / 32 / 24 B for
+                                                                # 3-D points / 3-D boxes / 5-D points; ours pads to 16 B)
+    npass = sort_passes(n, D)                                   # 8-bit digit passes, build sort
     qpass = (D * min(16, 32 // D) + 7) // 8                     # 8-bit digit passes, query sort
     nbatches = 3 if cfg["k"] else 2                             # query batches per step
     pairs = totals["pairs"]
-    tree = 4 * (n * lw + (n - 1) * nw)                          # tree read once by a traversal
+    per_touched = 4 * lw + 8 * D + 8                            # leaf + child box + links
+    tree_sp = per_touched * totals.get("touched_spatial", n)
+    tree_knn = per_touched * totals.get("touched_knn", n)
     b = {
         "B1_bounds": 4 * pw * n,
         "B2_codes": 4 * pw * n + 8 * n,
@@ -77,9 +94,8 @@ def algorithmic_bytes(cfg, totals):
         # pass 0 reads keys only (values are positions), later passes read and write (key,val)
         "B3_sort_pass": (8 + 12) * n + (npass - 1) * 24 * n,
         "B4_leaves": 4 * n + 4 * pw * n + 4 * lw * n,
-        # codes 8, leaf read, flag RMW 8, child box+ref write and read by the second arrival
-        "B5B6_hierarchy_refit": n * (8 + 4 * lw + 8) + (n - 1) * 2 * 4 * nw,
-        "Q1_qcodes": nbatches * 0,   # filled below per batch
+        # B5: codes 8 + links 8 + parent 4; B6: leaf read + flag RMW 8 + box write + box read by the parent
+        "B5B6_hierarchy_refit": n * (20 + 4 * lw + 8 + 16 * D),
         "T2_scan": 4 * nq + 4 * nq + 4 * (nq + 1),
     }
     q1_spatial = 4 * qw * nq + 4 * nq
@@ -87,28 +103,30 @@ def algorithmic_bytes(cfg, totals):
     b["Q1_qcodes"] = 2 * q1_spatial + (q1_knn if cfg["k"] else 0)
     b["Q2_qsort_hist"] = nbatches * 4 * nq
     b["Q2_qsort_pass"] = nbatches * ((4 + 8) * nq + (qpass - 1) * 16 * nq)
-    # traversal: order 4 + query row + result; the tree is read once per traversal
-    per_count = nq * (4 + 4 * qw + 4) + tree
+    # traversal: order 4 + query row + count 4; the reachable part of the tree once per traversal
+    per_count = nq * (4 + 4 * qw + 4) + tree_sp
     # arbx_query_count: one count traversal; arbx_query_spatial: one traversal that also stores
     # the hits in scratch rows (both under the T1 id), then the rows are copied into the CSR
     # slices (T3 id: rows read + indices written + counts and offsets read)
     b["T1_spatial_count"] = per_count + (per_count + 4 * pairs)
     b["T3_spatial_fill"] = 4 * pairs + 4 * pairs + 8 * nq
     if cfg["k"]:
-        b["K1K2_knn"] = nq * (4 + 4 * D + 8 * cfg["k"]) + tree
+        b["K1K2_knn"] = nq * (4 + 4 * D + 8 * cfg["k"]) + tree_knn
+    nw = 4 * (D + 1)
+    b["_whole_tree"] = 4 * (n * lw + (n - 1) * nw)
     return b
 
 
 # kernel id -> substring of the CUDA kernel name in the committed ncu launch list
-_NCU_KERNEL = {"K1K2_knn": "knn_thread_kernel", "T1_spatial_count": "spatial_kernel", "T3_spatial_fill": "compact_rows",
+_NCU_KERNEL = {"K1K2_knn": "knn_", "T1_spatial_count": "spatial_kernel", "T3_spatial_fill": "compact_rows",
                "B5B6_hierarchy_refit": "hierarchy_kernel", "B3_sort_pass": "onesweep_pass<unsigned long long",
                "Q2_qsort_pass": "onesweep_pass<unsigned int"}
 
 
 def ncu_traffic(kernel_id: str, workload: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-    committed ncu capture of this same workload (profiles/r1_launches_C3.csv); None if absent."""
-    path = os.path.join(ROOT, "profiles", f"r1_launches_{workload}.csv")
+    committed ncu capture of this same workload (profiles/r2_launches_<workload>.csv); None if absent."""
+    path = os.path.join(ROOT, "profiles", f"r2_launches_{workload}.csv")
     pat = _NCU_KERNEL.get(kernel_id)
     if not pat or not os.path.exists(path):
         return None
@@ -217,11 +235,14 @@ class ClockSampler:
 # ---- the oracle, timed (cpu_baseline leg and --impl reference) ----------------------------------
 def oracle_step(cfg, sample: int):
     """One bounded oracle 'step': grid build(s) over all N primitives + `sample` queries of each
-    batch kind.  Returns (seconds extrapolated to the full step, detail)."""
+    batch kind (sample >= Q: the whole step, nothing extrapolated).  Returns (seconds of the full
+    step -- extrapolated linearly in the number of queries when sample < Q --, full-step
+    queries/s, detail incl. the wall time this call really took)."""
     import oracle
     prims, pk = cfg["prims"], cfg["pkind"]
     nq = cfg["nq"]
     s = min(sample, nq)
+    t_begin = time.perf_counter()
     t0 = time.perf_counter()
     grid = oracle.Grid(prims, pk, oracle.default_cell(prims, pk, "spatial", cfg["r"] if cfg["r"] else None))
     t_build = time.perf_counter() - t0
@@ -241,9 +262,11 @@ def oracle_step(cfg, sample: int):
         oracle.knn(prims, pk, cfg["qpoints"][:s], cfg["k"], kgrid)
         t_knn = time.perf_counter() - t0
         del kgrid
+    wall = time.perf_counter() - t_begin
     nb = 3 if cfg["k"] else 2
     full = t_build + t_kbuild + (nq / s) * (t_spatial + t_count + t_knn)
-    detail = dict(sample_queries_per_batch=s, t_grid_build_s=round(t_build + t_kbuild, 3),
+    detail = dict(sample_queries_per_batch=s, extrapolated=bool(s < nq), wall_s=round(wall, 3),
+                  t_grid_build_s=round(t_build + t_kbuild, 3),
                   t_spatial_s=round(t_spatial, 3), t_count_s=round(t_count, 3), t_knn_s=round(t_knn, 3),
                   build_mprims_s=round(cfg["n"] / max(t_build, 1e-9) / 1e6, 3),
                   radius_qps=round(s / max(t_spatial, 1e-9), 1),
@@ -251,31 +274,98 @@ def oracle_step(cfg, sample: int):
     return full, nb * nq / full, detail
 
 
+def bench_config(cfg):
+    """The `config` object of the JSON line: the workload only, identical in both arms."""
+    return dict(workload=cfg["name"], n=cfg["n"], nq=cfg["nq"], dim=cfg["dim"], k=cfg["k"], r=cfg["r"])
+
+
 def run_reference(args, cfg):
+    """Reference arm = the oracle as it stands on the host cores.  Every step builds the grids
+    over all N primitives and answers a bounded sample of each query batch; the LAST timed step
+    answers ALL queries (nothing extrapolated) unless --ref-no-full-step.  `value` is the
+    full-step rate: measured in that last step, else extrapolated linearly in the query count."""
     import oracle
     oracle.build()
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     cores = oracle.num_threads()
-    times, vals, detail = [], [], None
+    fulls, walls, detail, full_detail = [], [], None, None
+    t_run0 = time.perf_counter()
     for i in range(args.warmup + args.steps):
-        full, v, detail = oracle_step(cfg, args.ref_sample)
+        last = i == args.warmup + args.steps - 1
+        whole = last and not args.ref_no_full_step
+        full, v, d = oracle_step(cfg, cfg["nq"] if whole else args.ref_sample)
         if i >= args.warmup:
-            times.append(full); vals.append(v)
+            walls.append(d["wall_s"])
+            if whole:
+                full_detail = d
+                full_step_s = full
+            else:
+                fulls.append(full)
+                detail = d
     nb = 3 if cfg["k"] else 2
-    ms = 1e3 * float(np.mean(times))
-    value = nb * cfg["nq"] / (ms / 1e3)
-    sample = (f"per step: uniform-grid build over all {cfg['n']} primitives + first {detail['sample_queries_per_batch']} "
-              f"queries of each of the {nb} batches, query time extrapolated linearly to Q={cfg['nq']}")
+    if full_detail is not None:
+        step_s, src = full_step_s, "measured: the last timed step answered all queries"
+    else:
+        step_s, src = float(np.mean(fulls)), "extrapolated linearly from the sampled queries"
+    value = nb * cfg["nq"] / step_s
+    ms_wall = 1e3 * float(np.mean(walls))
+    d0 = detail or full_detail
+    sample = (f"per step: uniform-grid build over all {cfg['n']} primitives + first {d0['sample_queries_per_batch']} "
+              f"queries of each of the {nb} batches; value = full-step rate ({src})")
     line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
-                warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="f64", data="synthetic",
-                config=dict(workload=cfg["name"], n=cfg["n"], nq=cfg["nq"], dim=cfg["dim"], k=cfg["k"], r=cfg["r"]),
-                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample, detail=detail),
+                warmup=args.warmup, ms_per_step=ms_wall, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic", config=bench_config(cfg),
+                ms_per_full_step=1e3 * step_s, full_step_source=src,
+                extrapolated_from_queries=None if full_detail is not None else d0["sample_queries_per_batch"],
+                sampled_steps_extrapolated_ms=[round(1e3 * f, 1) for f in fulls],
+                run_wall_s=round(time.perf_counter() - t_run0, 1),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample,
+                                  detail=full_detail or detail),
                 e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
     print(json.dumps(line), flush=True)
+
+
+def quick_config(arbx, torch, dg, name, dev, stream, steps=5, warmup=3):
+    """One configuration, device-resident inputs, the same step as the headline (build + CSR
+    radius/box query + count-only + kNN), CUDA events around every C-ABI call; median of `steps`."""
+    cfg = dg.config(name, 1.0)
+    n, nq, D, k, pk, qk = cfg["n"], cfg["nq"], cfg["dim"], cfg["k"], cfg["pkind"], cfg["qkind"]
+    prims, queries = torch.from_numpy(cfg["prims"]).to(dev), torch.from_numpy(cfg["queries"]).to(dev)
+    qpoints = torch.from_numpy(cfg["qpoints"]).to(dev) if k else None
+    offsets = torch.empty(nq + 1, dtype=torch.int32, device=dev)
+    counts = torch.empty(nq, dtype=torch.int32, device=dev)
+    kidx = torch.empty((nq, k), dtype=torch.int32, device=dev) if k else None
+    kdist = torch.empty((nq, k), dtype=torch.float32, device=dev) if k else None
+    rec = []
+    with torch.cuda.stream(stream):
+        h = arbx.arbx_build(prims, D, pk, stream)
+        _, total = arbx.arbx_query_spatial(h, queries, nq, qk, offsets, None, 0, stream)
+        arbx.arbx_destroy(h, stream)
+        indices = torch.empty(max(int(total), 1), dtype=torch.int32, device=dev)
+        for i in range(warmup + steps):
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+            ev[0].record(stream)
+            h = arbx.arbx_build(prims, D, pk, stream); ev[1].record(stream)
+            arbx.arbx_query_spatial(h, queries, nq, qk, offsets, indices, int(total), stream); ev[2].record(stream)
+            arbx.arbx_query_count(h, queries, nq, qk, counts, stream); ev[3].record(stream)
+            if k:
+                arbx.arbx_query_knn(h, qpoints, nq, k, kidx, kdist, stream)
+            ev[4].record(stream)
+            arbx.arbx_destroy(h, stream)
+            if i >= warmup:
+                rec.append(ev)
+        torch.cuda.synchronize()
+    t = np.median(np.array([[e[j].elapsed_time(e[j + 1]) for j in range(4)] + [e[0].elapsed_time(e[4])] for e in rec]), axis=0)
+    out = dict(n=n, nq=nq, dim=D, k=k, ms_per_step=round(float(t[4]), 4), build_ms=round(float(t[0]), 4),
+               build_mprims_s=round(n / t[0] / 1e3, 2), radius_csr_qps=round(nq / t[1] * 1e3, 1),
+               count_only_qps=round(nq / t[2] * 1e3, 1), knn_qps=round(nq / t[3] * 1e3, 1) if k else None,
+               pairs=int(total), steps=steps, warmup=warmup)
+    del prims, queries, qpoints, offsets, counts, kidx, kdist, indices
+    torch.cuda.empty_cache()
+    return out
 
 
 def main():
@@ -288,11 +378,23 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0, help="shrink N and Q (debugging only; a scaled run is not a bench value)")
     ap.add_argument("--ref-sample", type=int, default=200_000, help="oracle queries per batch per step")
     ap.add_argument("--cpu-sample", type=int, default=500_000, help="cpu_baseline queries per batch")
+    ap.add_argument("--ref-no-full-step", action="store_true", help="reference arm: do not run the last step on all queries")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short C1/C2/C4/C5 runs after the timed region")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print(f"note: --warmup {args.warmup} < 3 breaks the timing rules; use >= 3 for a reportable number", file=sys.stderr)
+
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` outside torchrun: start the N ranks ourselves (one per GPU)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execvp(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                   f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+                                   "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
 
     from paper_2507_23700_b200 import datagen as dg
     rank = int(os.environ.get("RANK", "0"))
@@ -310,6 +412,8 @@ def main():
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    if torch.cuda.device_count() < world:
+        raise SystemExit(f"bench.py: {world} ranks but only {torch.cuda.device_count()} CUDA devices (one rank per GPU)")
     arbx.lib()   # fail loudly if the extension is missing
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
@@ -339,6 +443,7 @@ def main():
         arbx.arbx_destroy(h0, stream)
     capacity = int(total)
     indices = torch.empty(max(capacity, 1), dtype=torch.int32, device=dev)
+    touched = {}     # distinct primitives in the results: the part of the tree a traversal must read
     counts = torch.empty(nq, dtype=torch.int32, device=dev)
     kidx = torch.empty((nq, k), dtype=torch.int32, device=dev) if k else None
     kdist = torch.empty((nq, k), dtype=torch.float32, device=dev) if k else None
@@ -399,6 +504,15 @@ def main():
         sampler_box[0] = None
         clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     ms_total = e0.elapsed_time(e1)
+    seen = torch.zeros(n, dtype=torch.bool, device=dev)
+    if capacity:
+        seen[indices[:capacity].long()] = True
+    touched["touched_spatial"] = int(seen.sum())
+    if k:
+        seen.zero_()
+        seen[kidx.reshape(-1).clamp_(min=0).long()] = True
+        touched["touched_knn"] = int(seen.sum())
+    del seen
     calls = {}
     for (na, ea), (nb_, eb) in zip(marks[:-1], marks[1:]):
         if nb_ != "begin":
@@ -516,6 +630,18 @@ def main():
         h2d = h_prims.numel() * 4 + h_queries.numel() * 4 + (h_qpoints.numel() * 4 if k else 0)
         d2h = ho.numel() * 4 + capacity * 4 + hc.numel() * 4 + (hki.numel() * 8 if k else 0)
         assert int(ho[-1]) == capacity and int(hc.sum()) == capacity, "e2e results inconsistent"
+    # ---- the other BASELINE.json configurations, same process, after the timed region ------------------
+    others = None
+    if rank == 0 and world == 1 and not args.no_other_configs and args.scale == 1.0:
+        del d_prims, d_queries, d_qpoints, indices, counts, kidx, kdist, offsets
+        if not args.no_e2e:
+            del inb, outb, ho, hi, hc, hki, hkd
+        torch.cuda.empty_cache()
+        others = {}
+        for name in ("C1", "C2", "C3", "C4", "C5"):
+            if name != cfg["name"]:
+                others[name] = quick_config(arbx, torch, dg, name, dev, stream)
+
     # max over ranks
     ms_step = ms_total / args.steps
     ms_step, ms_e2e_max = max_over_ranks([ms_step, ms_e2e if not args.no_e2e else 0.0], dev)
@@ -525,7 +651,7 @@ def main():
 
     if rank == 0:
         peak, peak_src = _peaks()
-        ab = algorithmic_bytes(cfg, dict(pairs=capacity))
+        ab = algorithmic_bytes(cfg, dict(pairs=capacity, **touched))
         kern = {}
         for name, (ms, ncalls) in prof.items():
             ms_s = ms / args.steps
@@ -551,7 +677,9 @@ def main():
             radius_csr_qps=round(nq / calls["spatial"] * 1e3, 1), radius_csr_ms=round(calls["spatial"], 4),
             count_only_qps=round(nq / calls["count"] * 1e3, 1), count_only_ms=round(calls["count"], 4),
             knn_qps=round(nq / calls["knn"] * 1e3, 1) if k else None, knn_ms=round(calls["knn"], 4) if k else None,
-            pairs=capacity, step_ms=step_stats, extras_outside_step=extras, kernels=kern)
+            pairs=capacity, step_ms=step_stats, extras_outside_step=extras, kernels=kern,
+            byte_model=dict(model="SURVEY.md 8(d) compulsory bytes; a traversal reads (leaf + child box + links) of the TOUCHED primitives once",
+                            whole_tree_bytes=int(ab["_whole_tree"]), **touched))
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             import oracle
@@ -564,11 +692,11 @@ def main():
         line = dict(metric=METRIC, value=world * nbatches * nq / (ms_step / 1e3), unit=UNIT, n_gpus=world,
                     steps=args.steps, warmup=args.warmup, ms_per_step=ms_step, higher_is_better=True,
                     scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
-                    config=dict(workload=cfg["name"], n=n, nq=nq, dim=D, k=k, r=cfg["r"], scale=args.scale,
-                                parallelism=f"replicas x{world}" if world > 1 else "single GPU",
-                                l2="inputs and outputs exceed L2 (no flush needed)" if (d_prims.numel() + d_queries.numel()) * 4 > 126e6 else "working set fits L2"),
+                    config=bench_config(cfg),
+                    run=dict(scale=args.scale, parallelism=f"replicas x{world}" if world > 1 else "single GPU",
+                             l2="inputs and outputs exceed L2 (no flush needed)" if (d_prims.numel() + d_queries.numel()) * 4 > 126e6 else "working set fits L2"),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline,
-                    cpu_baseline=cpu, breakdown=breakdown)
+                    cpu_baseline=cpu, breakdown=breakdown, other_configs=others)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -16,10 +16,13 @@
  *   pointers marked HOST are ordinary host memory.  The caller owns every buffer it passes;
  *   the library never returns device memory.  The handle owns the tree and a private copy
  *   of the geometry ("behave like a container"): `prims` may be released once
- *   the build has completed on `stream`.  Per-call scratch is taken from the CUDA
- *   stream-ordered allocator on `stream` and released before the call returns (in stream
- *   order); nothing per-query is stored in the handle, so several queries may run
- *   concurrently on one handle from different streams.
+ *   the build has completed on `stream`.  The tree and all per-call scratch come from a
+ *   stream-ordered memory pool that the library creates for itself on each device (the
+ *   process's default pool and the caller's allocator are not touched); scratch is released
+ *   before the call returns (in stream order) and stays cached in that pool up to 16 GiB
+ *   (arbx_trim hands the cache back to the driver).  Nothing per-query is stored in the
+ *   handle, so several queries may run concurrently on one handle from different streams
+ *   (PAPER.md:L77, L128).
  *   Using a handle on another stream than the one it was built on requires the caller to
  *   order that stream after the build (event or synchronize).
  *
@@ -146,22 +149,51 @@ ARBX_API arbx_status arbx_dbscan(arbx_handle h, float eps, int32_t min_pts, int3
 /* k nearest primitives to each query point ("a pair of a query point and a
  * number of neighbors"; L79 distance to the stored geometry: point ||x-y||, box point-box
  * distance (0 inside), sphere max(0,||y-c||-R)).  qpoints: DEVICE nq*dim.  One k per call,
- * 1 <= k <= ARBX_K_MAX.  indices: DEVICE int32[nq*k]; distances: DEVICE fp32[nq*k] or NULL.
+ * 1 <= k <= ARBX_K_MAX.  indices: DEVICE int32[nq*k]; distances: DEVICE fp32[nq*k] or NULL;
+ * both need only their natural 4-byte alignment.
  * Row q holds min(k,n) neighbours by ascending Euclidean distance (not squared); ties in
  * unspecified order; when n < k the row is padded with index -1 / distance +inf.
  * Asynchronous on `stream`.                                                                 */
 ARBX_API arbx_status arbx_query_knn(arbx_handle h, const float* qpoints, int64_t nq, int k,
                            int32_t* indices, float* distances, arbx_stream stream);
 
+/* As arbx_query_knn with one k per query (a nearest query IS "a pair of a query
+ * point and a number of neighbors").  k_per_query: DEVICE int32[nq], values clamped to
+ * [0, kmax]; 1 <= kmax <= ARBX_K_MAX.  indices / distances: rows of kmax entries; row q holds
+ * min(k_q, n) neighbours in ascending distance, then padding (index -1 / distance +inf).
+ * Asynchronous on `stream`.                                                                  */
+ARBX_API arbx_status arbx_query_knn_var(arbx_handle h, const float* qpoints, int64_t nq,
+                               const int32_t* k_per_query, int kmax, int32_t* indices,
+                               float* distances, arbx_stream stream);
+
+/* Return the library's cached device memory on the current device to the driver, keeping at
+ * most keep_bytes (0 = everything not in use).  Does not touch live handles.                 */
+ARBX_API arbx_status arbx_trim(int64_t keep_bytes);
+
+/* Test / experiment hook: sets one internal knob for the whole process (the library reads no
+ * environment variable).  Keys: "leaf_max" (primitives per collapsed leaf range, 1..64,
+ * default 16; applies to later builds), "code_bits" (space-filling-code bits per axis, 0 =
+ * adapted to n), "brute_max" (n at or below which arbx_build makes a brute-force index, -1 =
+ * default), "store_budget_mb" (scratch rows of the single-traversal storage query; 0 forces
+ * count -> scan -> fill), "traversal" (0 = per-warp choice, 1 = one query per lane, 2 =
+ * warp packets), "packet_alpha" (packet threshold, < 0 = default), "qbits" (query-code bits
+ * per axis used by the query sort, 0 = all), "l2_persist" (1 = persisting-L2 window over the
+ * node array during queries), "pool_keep_mb" (release threshold of the memory pool),
+ * "reset" (all knobs back to their defaults).  Results never depend on these knobs; they
+ * choose between equivalent paths.  ARBX_ERR_INVALID_ARG for an unknown key.                 */
+ARBX_API arbx_status arbx_debug_set(const char* key, double value);
+
 /* Stable LSD radix sort of (key, value) pairs, exposed for tests of build step B3
  * ("Sorting in both construction and search").  keys: DEVICE, sorted in place
- * on bits [0, key_bits); values: DEVICE uint32[n] or NULL (then only keys are sorted).
- * key_bytes is 4 or 8.  Asynchronous on `stream`.                                           */
+ * on bits [0, key_bits) -- bits at or above key_bits do not influence the order; values:
+ * DEVICE uint32[n] or NULL (then only keys are sorted).  key_bytes is 4 or 8.  Asynchronous
+ * on `stream`.                                                                              */
 ARBX_API arbx_status arbx_sort_pairs(void* keys, uint32_t* values, int64_t n, int key_bytes, int key_bits,
                             arbx_stream stream);
 
 /* Structural self-check of the tree (test hook for SURVEY.md §8(c-5) pin P9): verifies on
- * the device that sorted codes are non-decreasing, the leaf permutation is a permutation,
+ * the device that the build raised no fault, the space-filling codes of the leaves
+ * (recomputed from the leaf records) are non-decreasing, the leaf permutation is a permutation,
  * every node is reachable exactly once from the root, every stored child box equals the
  * union of that child's contents bit for bit.  *violations_host (HOST) = number of failed
  * checks (0 = valid).  Synchronises `stream`.                                               */

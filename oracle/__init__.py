@@ -131,6 +131,19 @@ def knn(prims, pkind: int, qpoints, k: int, grid: Grid | None = None):
     return idx, dist
 
 
+def knn_var(prims, pkind: int, qpoints, kq, kmax: int, grid: Grid | None = None):
+    """Per-query k (a nearest query is "a pair of a query point and a number of
+    neighbors"): row q holds the k_q = clip(kq[q], 0, kmax) nearest primitives, i.e. the first
+    k_q entries of the kmax-nearest row (rows ascend, ties by lower index), then padding
+    (-1 / +inf).  Returns (indices int32[nq,kmax], distances float64[nq,kmax])."""
+    idx, dist = knn(prims, pkind, qpoints, kmax, grid)
+    kq = np.clip(np.asarray(kq, dtype=np.int64), 0, kmax)
+    cut = np.arange(kmax)[None, :] >= kq[:, None]
+    idx[cut] = -1
+    dist[cut] = np.inf
+    return idx, dist
+
+
 def knn_distance_pairs(prims, pkind: int, qpoints, qids, pids) -> np.ndarray:
     """fp64 kNN distance of named (query, primitive) pairs (comparator rule 4)."""
     prims = _f32(prims)

@@ -202,3 +202,28 @@ def compare_dbscan(orc, labels, what: str = "") -> dict:
         else:
             assert labels[i] == -1, f"{what}: noise point {i} has label {labels[i]}"
     return dict(clusters=len(pairs), core=int(core.sum()), border=nborder, noise=int(n - core.sum() - nborder))
+
+
+def compare_knn_var(prims, pkind: int, qpoints, kq, kmax: int, orc, got, eps: float = EPS, what: str = "") -> None:
+    """Per-query k: orc / got are rows of kmax entries.  Queries are grouped by their k_q; the
+    first k_q columns of each group go through compare_knn with k = k_q, and every later column
+    must be padding (-1 / +inf)."""
+    o_idx, o_d = orc
+    g_idx, g_d = got
+    g_idx = np.asarray(g_idx)
+    nq = o_idx.shape[0]
+    assert g_idx.shape == (nq, kmax), f"{what}: shape {g_idx.shape} != {(nq, kmax)}"
+    kq = np.clip(np.asarray(kq, dtype=np.int64), 0, kmax)
+    cols = np.arange(kmax)[None, :]
+    pad = cols >= kq[:, None]
+    assert np.all(g_idx[pad] == -1), f"{what}: entries past k_q must be -1"
+    if g_d is not None:
+        assert np.all(np.isposinf(np.asarray(g_d)[pad])), f"{what}: distances past k_q must be +inf"
+    for kv in np.unique(kq):
+        if kv == 0:
+            continue
+        sel = np.nonzero(kq == kv)[0]
+        compare_knn(prims, pkind, np.ascontiguousarray(qpoints[sel]), int(kv),
+                    (np.ascontiguousarray(o_idx[sel, :kv]), np.ascontiguousarray(o_d[sel, :kv])),
+                    (np.ascontiguousarray(g_idx[sel, :kv]), None if g_d is None else np.ascontiguousarray(np.asarray(g_d)[sel, :kv])),
+                    eps=eps, what=f"{what} k_q={kv}")

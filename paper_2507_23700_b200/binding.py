@@ -24,6 +24,7 @@ LIB_PATH = os.path.join(_HERE, "libarbx.so")
 EXPORTS = (
     "arbx_build", "arbx_destroy", "arbx_size", "arbx_bounds", "arbx_query_count",
     "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_spatial_upto", "arbx_query_pairs", "arbx_dbscan", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
+    "arbx_query_knn_var", "arbx_trim", "arbx_debug_set",
     "arbx_launch_count", "arbx_profile_enable", "arbx_profile_num_kernels",
     "arbx_profile_kernel_name", "arbx_profile_read", "arbx_status_string", "arbx_last_error",
 )
@@ -60,6 +61,9 @@ def lib() -> ctypes.CDLL:
         L.arbx_query_pairs.argtypes = [vp, ctypes.c_float, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.arbx_dbscan.argtypes = [vp, ctypes.c_float, i32, vp, vp]
         L.arbx_query_knn.argtypes = [vp, vp, i64, i32, vp, vp, vp]
+        L.arbx_query_knn_var.argtypes = [vp, vp, i64, vp, i32, vp, vp, vp]
+        L.arbx_trim.argtypes = [i64]
+        L.arbx_debug_set.argtypes = [ctypes.c_char_p, ctypes.c_double]
         L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
         L.arbx_debug_validate.argtypes = [vp, ctypes.POINTER(i64), vp]
         L.arbx_launch_count.restype = i64
@@ -73,7 +77,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_status_string.restype = ctypes.c_char_p
         L.arbx_status_string.argtypes = [i32]
         L.arbx_last_error.restype = ctypes.c_char_p
-        for name in EXPORTS[:13]:
+        for name in EXPORTS[:16]:
             getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -189,6 +193,23 @@ def arbx_query_knn(handle: int, qpoints: torch.Tensor, nq: int, k: int, indices:
            "arbx_query_knn")
 
 
+def arbx_query_knn_var(handle: int, qpoints: torch.Tensor, nq: int, k_per_query: torch.Tensor, kmax: int,
+                       indices: torch.Tensor, distances, stream=None) -> None:
+    if not (k_per_query.is_cuda and k_per_query.dtype == torch.int32 and k_per_query.is_contiguous()):
+        raise TypeError("k_per_query must be a contiguous CUDA int32 tensor")
+    _check(lib().arbx_query_knn_var(handle, _ptr(qpoints), nq, _ptr(k_per_query), kmax, _ptr(indices),
+                                    0 if distances is None else _ptr(distances), _stream(stream)),
+           "arbx_query_knn_var")
+
+
+def arbx_trim(keep_bytes: int = 0) -> None:
+    _check(lib().arbx_trim(keep_bytes), "arbx_trim")
+
+
+def arbx_debug_set(key: str, value: float) -> None:
+    _check(lib().arbx_debug_set(key.encode(), float(value)), "arbx_debug_set")
+
+
 def arbx_sort_pairs(keys: torch.Tensor, values, key_bits: int, stream=None) -> None:
     assert keys.is_cuda and keys.is_contiguous() and keys.element_size() in (4, 8)
     _check(lib().arbx_sort_pairs(_ptr(keys), 0 if values is None else _ptr(values), keys.numel(),
@@ -232,6 +253,7 @@ class Index:
             dim = w if kind == POINT else w // 2 if kind == BOX else w - 1
         self.dim, self.kind, self.device = dim, kind, prims.device
         self.handle = arbx_build(prims, dim, kind, stream)
+        self._per_query = 16.0      # matches per query seen so far: sizes the next CSR buffer
 
     def close(self, stream=None):
         if getattr(self, "handle", None):
@@ -270,19 +292,21 @@ class Index:
 
     def query_spatial(self, queries: torch.Tensor, qkind: int = SPHERE, capacity: int | None = None,
                       stream=None):
-        """CSR result (offsets int32[nq+1], indices int32[total]).  With `capacity` (an upper
-        bound the caller knows) the whole query is one ABI call; otherwise a first call with
-        indices=NULL learns the total (count + scan) and a second call fills."""
+        """CSR result (offsets int32[nq+1], indices int32[total]).  One ABI call (one traversal)
+        when `capacity` -- given by the caller, else guessed from the matches per query this
+        index has seen so far -- holds the result; on ARBX_ERR_CAPACITY the call has left the
+        exact total, and a second call with a buffer of that size fills."""
         nq = self._nq(queries, qkind)
         offsets = torch.empty(nq + 1, dtype=torch.int32, device=self.device)
-        if capacity is not None:
-            indices = torch.empty(capacity, dtype=torch.int32, device=self.device)
-            st, total = arbx_query_spatial(self.handle, queries, nq, qkind, offsets, indices, capacity,
-                                           stream, raise_on_capacity=False)
-            if st == OK:
-                return offsets, indices[:total]
-        else:
-            _, total = arbx_query_spatial(self.handle, queries, nq, qkind, offsets, None, 0, stream)
+        if capacity is None:
+            capacity = int(nq * self._per_query * 1.25) + 1024
+        indices = torch.empty(capacity, dtype=torch.int32, device=self.device)
+        st, total = arbx_query_spatial(self.handle, queries, nq, qkind, offsets, indices, capacity,
+                                       stream, raise_on_capacity=False)
+        if nq:
+            self._per_query = max(1.0, total / nq)
+        if st == OK:
+            return offsets, indices[:total]
         indices = torch.empty(total, dtype=torch.int32, device=self.device)
         arbx_query_spatial(self.handle, queries, nq, qkind, offsets, indices, total, stream)
         return offsets, indices
@@ -311,11 +335,19 @@ class Index:
         arbx_dbscan(self.handle, eps, min_pts, labels, stream)
         return labels
 
-    def query_knn(self, qpoints: torch.Tensor, k: int, want_distances: bool = True, stream=None):
+    def query_knn(self, qpoints: torch.Tensor, k, want_distances: bool = True, stream=None, kmax: int | None = None):
+        """k: one int for all queries, or a CUDA int32 tensor with one k per query (rows of kmax
+        entries, padded with -1 / +inf; kmax defaults to max(k))."""
         nq = self._nq(qpoints, POINT)
-        idx = torch.empty((nq, k), dtype=torch.int32, device=self.device)
-        dist = torch.empty((nq, k), dtype=torch.float32, device=self.device) if want_distances else None
-        arbx_query_knn(self.handle, qpoints, nq, k, idx, dist, stream)
+        per_query = isinstance(k, torch.Tensor)
+        width = int(k) if not per_query else int(kmax if kmax is not None else (int(k.max()) if nq else 1))
+        width = max(width, 1)
+        idx = torch.empty((nq, width), dtype=torch.int32, device=self.device)
+        dist = torch.empty((nq, width), dtype=torch.float32, device=self.device) if want_distances else None
+        if per_query:
+            arbx_query_knn_var(self.handle, qpoints, nq, k, width, idx, dist, stream)
+        else:
+            arbx_query_knn(self.handle, qpoints, nq, width, idx, dist, stream)
         return idx, dist
 
     def validate(self, stream=None) -> int:

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <mutex>
+#include <string>
 #include <vector>
 
 #include "common.cuh"
@@ -16,6 +17,7 @@
 namespace arbx {
 
 std::atomic<long long> g_launches{0};
+DebugCfg g_cfg;
 static thread_local char t_err[512] = "";
 
 void set_error(const char* fmt, ...) {
@@ -60,28 +62,57 @@ void prof_end(int id, cudaStream_t s) {
     }
 }
 
+// Device memory (the handle's tree and all per-call scratch) comes from a stream-ordered pool
+// OWNED BY THE LIBRARY, one per device: the process-wide default pool and PyTorch's caching
+// allocator are left alone.  Freed blocks stay cached in the pool up to a bounded release
+// threshold (so that the host synchronisation inside the storage query does not hand the
+// scratch back to the driver every call); arbx_trim returns the cache to the driver.
 static std::once_flag g_pool_once[64];
+static cudaMemPool_t g_pool[64];
+static std::atomic<long long> g_pool_keep_mb{16384};
+static std::atomic<int> g_pool_thr_set[64];
+
+static void pool_apply_threshold(cudaMemPool_t pool) {
+  unsigned long long thr = (unsigned long long)g_pool_keep_mb.load() << 20;
+  if (cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr) != cudaSuccess) cudaGetLastError();
+}
+
+static cudaMemPool_t pool_for(int dev) {
+  if (dev < 0 || dev >= 64) return nullptr;
+  std::call_once(g_pool_once[dev], [dev] {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t pool = nullptr;
+    if (cudaMemPoolCreate(&pool, &props) == cudaSuccess) {
+      pool_apply_threshold(pool);
+      g_pool[dev] = pool;
+    } else {
+      cudaGetLastError();
+      g_pool[dev] = nullptr;
+    }
+  });
+  return g_pool[dev];
+}
 
 arbx_status scratch_alloc(void** p, size_t bytes, cudaStream_t s) {
   int dev = 0;
   cudaGetDevice(&dev);
-  if (dev >= 0 && dev < 64) {
-    // keep freed scratch cached in the stream-ordered pool instead of returning it to the OS
-    std::call_once(g_pool_once[dev], [dev] {
-      cudaMemPool_t pool;
-      if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-        unsigned long long thr = ~0ull;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-      }
-    });
-  }
+  cudaMemPool_t pool = pool_for(dev);
   *p = nullptr;
-  cudaError_t e = cudaMallocAsync(p, bytes ? bytes : 1, s);
+  if (!pool) { set_error("could not create the library's memory pool on device %d", dev); return ARBX_ERR_CUDA; }
+  cudaError_t e = cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, s);
   if (e != cudaSuccess) {
     cudaGetLastError();
-    set_error("cudaMallocAsync(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
+    set_error("cudaMallocFromPoolAsync(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
     return e == cudaErrorMemoryAllocation ? ARBX_ERR_OOM : ARBX_ERR_CUDA;
   }
+  // measured on B200 / CUDA 12.9: a release threshold set on a pool that has never allocated is
+  // not honoured (every synchronisation hands the cache back: 7.8 -> 35 ms per C4 step), so it is
+  // applied again after the pool's first allocation
+  if (!g_pool_thr_set[dev].exchange(1)) pool_apply_threshold(pool);
   return ARBX_OK;
 }
 void scratch_free(void* p, cudaStream_t s) { if (p) cudaFreeAsync(p, s); }
@@ -101,25 +132,69 @@ const DimTable* dim_table(int dim) {
   return nullptr;
 }
 
-static int env_int(const char* name, int dflt) {
-  const char* v = getenv(name);
-  return v && *v ? atoi(v) : dflt;
-}
-
 static void free_index(Index* ix, cudaStream_t s) {
   scratch_free(ix->leaves, s); scratch_free(ix->nodes, s); scratch_free(ix->bounds, s);
-  scratch_free(ix->root, s); scratch_free(ix->codes, s);
+  scratch_free(ix->root, s);
 }
 
 // Q1 + Q2: order in which the queries are traversed (neighbours on the curve share a warp)
+struct QueryOrder {
+  Scratch<uint32_t> buf[2];
+  const uint32_t* p = nullptr;   // order[t] = caller's index of the t-th query on the curve
+};
 static arbx_status query_order(const Index* ix, const float* queries, int64_t nq, int qkind,
-                               Scratch<uint32_t>& order, cudaStream_t s) {
-  Scratch<uint32_t> codes;
+                               QueryOrder& order, cudaStream_t s) {
+  if (ix->brute) { order.p = nullptr; return ARBX_OK; }   // every query scans every primitive: order is irrelevant
+  Scratch<uint32_t> codes, codes_alt;
   ARBX_TRY(codes.alloc((size_t)nq, s));
-  ARBX_TRY(order.alloc((size_t)nq, s));
+  ARBX_TRY(codes_alt.alloc((size_t)nq, s));
+  ARBX_TRY(order.buf[0].alloc((size_t)nq, s));
+  ARBX_TRY(order.buf[1].alloc((size_t)nq, s));
   int key_bits = 32;
   ARBX_TRY(dim_table(ix->dim)->qcode(ix, queries, nq, qkind, codes.p, &key_bits, s));
-  return radix_sort_u32(codes.p, order.p, true, nq, key_bits, s);
+  uint32_t *kout = nullptr, *vout = nullptr;
+  ARBX_TRY(radix_sort_u32(codes.p, codes_alt.p, order.buf[0].p, order.buf[1].p, true, nq, key_bits, s, &kout, &vout));
+  order.p = vout;
+  return ARBX_OK;
+}
+
+// Experiment (knob "l2_persist"): a persisting-L2 access-policy window over the node array for
+// the kernels of one query call.  Node ids are split positions, so the upper levels are NOT
+// contiguous: the window can only cover the whole array with hitRatio = carve-out / size.
+struct L2Window {
+  cudaStream_t s; bool on = false;
+  L2Window(const Index* ix, cudaStream_t s_) : s(s_) {
+    if (!g_cfg.l2_persist.load(std::memory_order_relaxed) || !ix->nodes || ix->n < 2) return;
+    int dev = 0, max_persist = 0, max_window = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
+    cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
+    if (max_persist <= 0 || max_window <= 0) return;
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)max_persist);
+    const size_t bytes = std::min<size_t>((size_t)(ix->n - 1) * node_width(ix->dim) * sizeof(float), (size_t)max_window);
+    cudaStreamAttrValue v = {};
+    v.accessPolicyWindow.base_ptr = ix->nodes;
+    v.accessPolicyWindow.num_bytes = bytes;
+    v.accessPolicyWindow.hitRatio = std::min(1.0f, (float)max_persist / (float)bytes);
+    v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    v.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    on = cudaStreamSetAttribute(s, cudaStreamAttributeAccessPolicyWindow, &v) == cudaSuccess;
+    if (!on) cudaGetLastError();
+  }
+  ~L2Window() {
+    if (!on) return;
+    cudaStreamAttrValue v = {};
+    v.accessPolicyWindow.num_bytes = 0;
+    cudaStreamSetAttribute(s, cudaStreamAttributeAccessPolicyWindow, &v);
+  }
+};
+
+// A fault raised by the (asynchronous) build kernels is reported by the first call on the
+// handle that synchronises with the host.
+static arbx_status check_build_fault(int32_t flags) {
+  if (flags == 0) return ARBX_OK;
+  set_error("the build of this handle failed on the device (fault flags 0x%x: parked-subtree list overflow)", flags);
+  return ARBX_ERR_CUDA;
 }
 
 __global__ void fill_i32_kernel(int32_t* p, int64_t n, int32_t v) {
@@ -183,7 +258,7 @@ arbx_status arbx_build(const float* prims, int64_t n, int dim, arbx_kind kind, a
   if (n > kMaxCount) { set_error("arbx_build: n > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
   cudaStream_t s = (cudaStream_t)stream;
   arbx_index_s* h = new arbx_index_s();
-  h->ix.leaf_max = std::max(1, std::min(64, env_int("ARBX_LEAF_MAX", 16)));
+  h->ix.leaf_max = std::max(1, std::min(64, g_cfg.leaf_max.load(std::memory_order_relaxed)));
   arbx_status st = build_index(prims, n, dim, (int)kind, s, &h->ix);
   if (st != ARBX_OK) {
     free_index(&h->ix, s);
@@ -211,9 +286,12 @@ arbx_status arbx_bounds(arbx_handle h, float* lo_host, float* hi_host, arbx_stre
   if (!h || !lo_host || !hi_host) { set_error("arbx_bounds: null argument"); return ARBX_ERR_INVALID_ARG; }
   cudaStream_t s = (cudaStream_t)stream;
   float tmp[2 * ARBX_MAX_DIM];
+  int32_t rootw[2] = {0, 0};
   const int D = h->ix.dim;
   ARBX_CUDA(cudaMemcpyAsync(tmp, h->ix.bounds, 2 * D * sizeof(float), cudaMemcpyDeviceToHost, s));
+  ARBX_CUDA(cudaMemcpyAsync(rootw, h->ix.root, sizeof(rootw), cudaMemcpyDeviceToHost, s));
   ARBX_CUDA(cudaStreamSynchronize(s));
+  ARBX_TRY(check_build_fault(rootw[1]));
   for (int a = 0; a < D; ++a) { lo_host[a] = tmp[a]; hi_host[a] = tmp[D + a]; }
   return ARBX_OK;
 }
@@ -243,9 +321,10 @@ static arbx_status count_impl(arbx_handle h, const float* queries, int64_t nq, a
   cudaStream_t s = (cudaStream_t)stream;
   const Index* ix = &h->ix;
   if (ix->n == 0) { ARBX_CUDA(cudaMemsetAsync(counts, 0, (size_t)nq * sizeof(int32_t), s)); return ARBX_OK; }
-  Scratch<uint32_t> order;
+  QueryOrder order;
   ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
   SpatialArgs a{queries, nq, (int)qkind, order.p, counts, nullptr, nullptr, nullptr, limit, nullptr, 0};
+  L2Window l2(ix, s);
   return dim_table(ix->dim)->spatial(ix, a, s);
 }
 
@@ -285,7 +364,7 @@ arbx_status arbx_dbscan(arbx_handle h, float eps, int32_t min_pts, int32_t* labe
   cudaStream_t s = (cudaStream_t)stream;
   const unsigned grid = (unsigned)((n + 255) / 256);
   Scratch<float> selfq;
-  Scratch<uint32_t> order;
+  Scratch<uint32_t> order;   // tree order is the traversal order: no query sort
   Scratch<int32_t> counts, uf;
   ARBX_TRY(selfq.alloc((size_t)n * (ix->dim + 1), s));
   ARBX_TRY(order.alloc((size_t)n, s));
@@ -327,20 +406,22 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
     ARBX_CUDA(cudaMemsetAsync(offsets, 0, (size_t)(nq + 1) * sizeof(int32_t), s));
     return ARBX_OK;
   }
-  Scratch<uint32_t> order;
+  QueryOrder order;
   Scratch<int32_t> counts, rows;
   Scratch<long long> total_dev;   // [0] total, [1] number of queries with more than `cap` matches
   Scratch<float> selfq;
   if (self) {
     ARBX_TRY(selfq.alloc((size_t)nq * (ix->dim + 1), s));
-    ARBX_TRY(order.alloc((size_t)nq, s));
+    ARBX_TRY(order.buf[0].alloc((size_t)nq, s));
     self_queries_kernel<<<(unsigned)((nq + 255) / 256), 256, 0, s>>>(ix->leaves, nq, ix->dim, leaf_width(KIND_POINT, ix->dim),
-                                                                  self_radius, selfq.p, order.p);
+                                                                  self_radius, selfq.p, order.buf[0].p);
     ARBX_LAUNCH_CHECK();
+    order.p = order.buf[0].p;
     queries = selfq.p;
   } else {
     ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
   }
+  L2Window l2(ix, s);
   ARBX_TRY(counts.alloc((size_t)nq, s));
   ARBX_TRY(total_dev.alloc(2, s));
   ARBX_CUDA(cudaMemsetAsync(total_dev.p, 0, 2 * sizeof(long long), s));
@@ -350,7 +431,7 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
   // their CSR slices and only queries with more than cap matches are traversed again.
   int cap = 0;
   if (indices && limit == 0) {
-    const long long budget = (long long)env_int("ARBX_STORE_BUDGET_MB", 4096) << 20;
+    const long long budget = (long long)g_cfg.store_budget_mb.load(std::memory_order_relaxed) << 20;
     for (int c = 64; c >= 16 && cap == 0; c >>= 1)
       if ((long long)nq * c * 4 <= budget) cap = c;
   }
@@ -366,8 +447,11 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
   ARBX_TRY(tab->spatial(ix, a, s));
   ARBX_TRY(exclusive_scan_i32(counts.p, offsets, nq, total_dev.p, s));
   long long host[2] = {0, 0};
+  int32_t rootw[2] = {0, 0};
   ARBX_CUDA(cudaMemcpyAsync(host, total_dev.p, sizeof(host), cudaMemcpyDeviceToHost, s));
+  ARBX_CUDA(cudaMemcpyAsync(rootw, ix->root, sizeof(rootw), cudaMemcpyDeviceToHost, s));
   ARBX_CUDA(cudaStreamSynchronize(s));
+  ARBX_TRY(check_build_fault(rootw[1]));
   const long long total = host[0];
   const int noverflow = (int)(host[1] & 0xffffffffLL);
   if (total_host) *total_host = total;
@@ -392,14 +476,14 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
   return tab->spatial(ix, a, s);
 }
 
-arbx_status arbx_query_knn(arbx_handle h, const float* qpoints, int64_t nq, int k, int32_t* indices,
-                           float* distances, arbx_stream stream) {
+static arbx_status knn_impl(arbx_handle h, const float* qpoints, int64_t nq, const int32_t* kq, int k,
+                            int32_t* indices, float* distances, arbx_stream stream, const char* who) {
   if (!h || nq < 0 || k < 1 || (nq > 0 && (!qpoints || !indices))) {
-    set_error("arbx_query_knn: invalid argument");
+    set_error("%s: invalid argument", who);
     return ARBX_ERR_INVALID_ARG;
   }
-  if (k > ARBX_K_MAX) { set_error("arbx_query_knn: k=%d > ARBX_K_MAX=%d", k, ARBX_K_MAX); return ARBX_ERR_UNSUPPORTED; }
-  if (nq > kMaxCount) { set_error("arbx_query_knn: nq > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
+  if (k > ARBX_K_MAX) { set_error("%s: k=%d > ARBX_K_MAX=%d", who, k, ARBX_K_MAX); return ARBX_ERR_UNSUPPORTED; }
+  if (nq > kMaxCount) { set_error("%s: nq > 2^30 unsupported", who); return ARBX_ERR_UNSUPPORTED; }
   if (nq == 0) return ARBX_OK;
   cudaStream_t s = (cudaStream_t)stream;
   const Index* ix = &h->ix;
@@ -408,9 +492,22 @@ arbx_status arbx_query_knn(arbx_handle h, const float* qpoints, int64_t nq, int 
     ARBX_LAUNCH_CHECK();
     return ARBX_OK;
   }
-  Scratch<uint32_t> order;
+  QueryOrder order;
   ARBX_TRY(query_order(ix, qpoints, nq, KIND_POINT, order, s));
-  return dim_table(ix->dim)->knn(ix, qpoints, nq, k, order.p, indices, distances, s);
+  KnnArgs a{qpoints, nq, k, kq, order.p, indices, distances};
+  L2Window l2(ix, s);
+  return dim_table(ix->dim)->knn(ix, a, s);
+}
+
+arbx_status arbx_query_knn(arbx_handle h, const float* qpoints, int64_t nq, int k, int32_t* indices,
+                           float* distances, arbx_stream stream) {
+  return knn_impl(h, qpoints, nq, nullptr, k, indices, distances, stream, "arbx_query_knn");
+}
+
+arbx_status arbx_query_knn_var(arbx_handle h, const float* qpoints, int64_t nq, const int32_t* k_per_query,
+                               int kmax, int32_t* indices, float* distances, arbx_stream stream) {
+  if (nq > 0 && !k_per_query) { set_error("arbx_query_knn_var: null k_per_query"); return ARBX_ERR_INVALID_ARG; }
+  return knn_impl(h, qpoints, nq, k_per_query, kmax, indices, distances, stream, "arbx_query_knn_var");
 }
 
 arbx_status arbx_sort_pairs(void* keys, uint32_t* values, int64_t n, int key_bytes, int key_bits,
@@ -420,8 +517,67 @@ arbx_status arbx_sort_pairs(void* keys, uint32_t* values, int64_t n, int key_byt
     return ARBX_ERR_INVALID_ARG;
   }
   cudaStream_t s = (cudaStream_t)stream;
-  if (key_bytes == 8) return radix_sort_u64((unsigned long long*)keys, values, false, n, key_bits, s);
-  return radix_sort_u32((uint32_t*)keys, values, false, n, key_bits, s);
+  if (n == 0) return ARBX_OK;
+  Scratch<unsigned char> kalt;
+  Scratch<uint32_t> valt;
+  ARBX_TRY(kalt.alloc((size_t)n * key_bytes, s));
+  if (values) ARBX_TRY(valt.alloc((size_t)n, s));
+  void* kout = keys;
+  uint32_t* vout = values;
+  if (key_bytes == 8) {
+    unsigned long long* ko = nullptr;
+    ARBX_TRY(radix_sort_u64((unsigned long long*)keys, (unsigned long long*)kalt.p, values, valt.p, false, n, key_bits, s, &ko, &vout));
+    kout = ko;
+  } else {
+    uint32_t* ko = nullptr;
+    ARBX_TRY(radix_sort_u32((uint32_t*)keys, (uint32_t*)kalt.p, values, valt.p, false, n, key_bits, s, &ko, &vout));
+    kout = ko;
+  }
+  if (kout != keys) {   // odd number of passes: the result sits in the scratch buffers
+    ARBX_CUDA(cudaMemcpyAsync(keys, kout, (size_t)n * key_bytes, cudaMemcpyDeviceToDevice, s));
+    if (values) ARBX_CUDA(cudaMemcpyAsync(values, vout, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, s));
+  }
+  return ARBX_OK;
+}
+
+arbx_status arbx_debug_set(const char* key, double value) {
+  if (!key) { set_error("arbx_debug_set: null key"); return ARBX_ERR_INVALID_ARG; }
+  const std::string k(key);
+  const int iv = (int)value;
+  if (k == "leaf_max") g_cfg.leaf_max.store(iv);
+  else if (k == "store_budget_mb") g_cfg.store_budget_mb.store(iv);
+  else if (k == "traversal") g_cfg.traversal.store(iv);
+  else if (k == "qbits") g_cfg.qbits.store(iv);
+  else if (k == "code_bits") g_cfg.code_bits.store(iv);
+  else if (k == "brute_max") g_cfg.brute_max.store(iv);
+  else if (k == "l2_persist") g_cfg.l2_persist.store(iv);
+  else if (k == "packet_alpha") g_cfg.packet_alpha.store((float)value);
+  else if (k == "pool_keep_mb") {
+    g_pool_keep_mb.store((long long)value);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaMemPool_t pool = pool_for(dev)) pool_apply_threshold(pool);
+  } else if (k == "reset") {
+    g_cfg.leaf_max.store(16); g_cfg.store_budget_mb.store(4096); g_cfg.traversal.store(0); g_cfg.qbits.store(0);
+    g_cfg.code_bits.store(0); g_cfg.brute_max.store(-1); g_cfg.l2_persist.store(0); g_cfg.packet_alpha.store(-1.f);
+  } else {
+    set_error("arbx_debug_set: unknown key '%s'", key);
+    return ARBX_ERR_INVALID_ARG;
+  }
+  return ARBX_OK;
+}
+
+#ifdef ARBX_STATS
+extern "C++" { namespace arbx { void knn_stats_read(unsigned long long* out); } }
+extern "C" __attribute__((visibility("default"))) void arbx_debug_knn_stats(unsigned long long* out) { arbx::knn_stats_read(out); }
+#endif
+
+arbx_status arbx_trim(int64_t keep_bytes) {
+  if (keep_bytes < 0) { set_error("arbx_trim: keep_bytes < 0"); return ARBX_ERR_INVALID_ARG; }
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (cudaMemPool_t pool = pool_for(dev)) ARBX_CUDA(cudaMemPoolTrimTo(pool, (size_t)keep_bytes));
+  return ARBX_OK;
 }
 
 arbx_status arbx_debug_validate(arbx_handle h, int64_t* violations_host, arbx_stream stream) {

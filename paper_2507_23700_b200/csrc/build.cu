@@ -72,7 +72,7 @@ __global__ void bounds_decode_kernel(const uint32_t* enc, float* bounds, int D) 
 template <int D, int PK>
 __global__ void __launch_bounds__(BT) codes_kernel(const float* __restrict__ prims, int64_t n,
                                                    const float* __restrict__ bounds,
-                                                   unsigned long long* __restrict__ codes) {
+                                                   unsigned long long* __restrict__ codes, int drop) {
   constexpr int W = prim_width(PK, D);
   constexpr int B = code_bits_per_axis(D);
   float lo[D], scale[D];
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(BT) codes_kernel(const float* __restrict__ pri
     centre_of<D, PK>(v, c);
     uint32_t q[D];
     quantise<D, B>(c, lo, scale, q);
-    codes[i] = interleave<D, B, unsigned long long>(q);
+    codes[i] = interleave<D, B, unsigned long long>(q) >> drop;   // keep the top bits of every axis
   }
 }
 
@@ -107,6 +107,28 @@ __global__ void __launch_bounds__(BT) leaves_kernel(const float* __restrict__ pr
 #pragma unroll
   for (int e = 0; e < W; ++e) v[e] = __ldg(prims + (int64_t)i * W + e);
   v[W] = __uint_as_float(i);
+#pragma unroll
+  for (int e = W + 1; e < LW; ++e) v[e] = 0.f;
+  float4* out = reinterpret_cast<float4*>(leaves + j * LW);
+#pragma unroll
+  for (int e = 0; e < LW / 4; ++e) out[e] = make_float4(v[4 * e], v[4 * e + 1], v[4 * e + 2], v[4 * e + 3]);
+}
+
+// Brute-force index ("new brute-force search structure"): the primitives in the
+// caller's order form ONE leaf range [0, n), root = ~0; the traversal kernels then scan every
+// primitive for every query, and no codes, sort or hierarchy are needed.
+template <int D, int PK>
+__global__ void __launch_bounds__(BT) brute_leaves_kernel(const float* __restrict__ prims, int64_t n,
+                                                          float* __restrict__ leaves, int32_t* __restrict__ root) {
+  constexpr int W = prim_width(PK, D);
+  constexpr int LW = leaf_width(PK, D);
+  const int64_t j = (int64_t)blockIdx.x * BT + threadIdx.x;
+  if (j == 0) root[0] = ~0;
+  if (j >= n) return;
+  float v[LW];
+#pragma unroll
+  for (int e = 0; e < W; ++e) v[e] = __ldg(prims + j * W + e);
+  v[W] = __uint_as_float((uint32_t)j | (j == n - 1 ? LEAF_END : 0u));
 #pragma unroll
   for (int e = W + 1; e < LW; ++e) v[e] = 0.f;
   float4* out = reinterpret_cast<float4*>(leaves + j * LW);
@@ -265,6 +287,8 @@ hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict
         open_lrf[3 * e] = l; open_lrf[3 * e + 1] = r; open_lrf[3 * e + 2] = ref;
 #pragma unroll
         for (int a = 0; a < D; ++a) { open_box[(int64_t)e * 2 * D + a] = lo[a]; open_box[(int64_t)e * 2 * D + D + a] = hi[a]; }
+      } else {
+        atomicOr(root + 1, BUILD_FAULT_OPEN_OVERFLOW);   // never silent: every query on this handle fails
       }
       return;
     }
@@ -338,7 +362,8 @@ template <int D, int PK>
 arbx_status build_typed(const float* prims, int64_t n, cudaStream_t s, Index* ix, int sms) {
   constexpr int LW = leaf_width(PK, D);
   constexpr int NW = node_width(D);
-  Scratch<uint32_t> enc, perm;
+  Scratch<uint32_t> enc, perm, perm_alt;
+  Scratch<unsigned long long> codes, codes_alt;
   Scratch<int> flags;
   ARBX_TRY(enc.alloc(2 * D, s));
   const int sgrid = grid_for(n, BT, sms * 8);
@@ -352,20 +377,52 @@ arbx_status build_typed(const float* prims, int64_t n, cudaStream_t s, Index* ix
     ARBX_LAUNCH_CHECK();
   }
 
-  ARBX_TRY(scratch_alloc((void**)&ix->codes, (size_t)n * sizeof(unsigned long long), s));
+  // Tiny inputs: a tree costs ~25 dependent launches to build and saves nothing at query time
+  int brute_max = g_cfg.brute_max.load(std::memory_order_relaxed);
+  if (brute_max < 0) brute_max = 512;
+  if (n <= brute_max) {
+    ix->brute = true;
+    ix->leaf_max = (int)std::max<int64_t>(n, 1);
+    ARBX_TRY(scratch_alloc((void**)&ix->leaves, (size_t)n * LW * sizeof(float), s));
+    ProfScope ps(K_LEAVES, s);
+    brute_leaves_kernel<D, PK><<<(unsigned)((n + BT - 1) / BT), BT, 0, s>>>(prims, n, ix->leaves, ix->root);
+    ARBX_LAUNCH_CHECK();
+    return ARBX_OK;
+  }
+
+  // Code width (reading A15): b bits per axis, b <= floor(64/D).  The tree shape is not
+  // observable in results and duplicate codes are split by sorted position (A16), so the codes
+  // only need to resolve the primitives: b = ceil(log2(n)/D) + 4 bits per axis (16^D cells per
+  // primitive on average), rounded up to fill whole 8-bit sort passes.
+  constexpr int BMAX = code_bits_per_axis(D);
+  int b = g_cfg.code_bits.load(std::memory_order_relaxed);
+  if (b <= 0) {
+    int lg = 0;
+    while ((int64_t(1) << lg) < n) ++lg;
+    b = (lg + D - 1) / D + 4;
+    const int passes = (D * b + 7) / 8;
+    b = std::max(b, 8 * passes / D);
+  }
+  b = std::max(1, std::min(BMAX, b));
+  ix->code_bits = b;
+  ARBX_TRY(codes.alloc((size_t)n, s));
+  ARBX_TRY(codes_alt.alloc((size_t)n, s));
   {
     ProfScope ps(K_CODES, s);
-    codes_kernel<D, PK><<<sgrid, BT, 0, s>>>(prims, n, ix->bounds, ix->codes);
+    codes_kernel<D, PK><<<sgrid, BT, 0, s>>>(prims, n, ix->bounds, codes.p, D * (BMAX - b));
     ARBX_LAUNCH_CHECK();
   }
   ARBX_TRY(perm.alloc((size_t)n, s));
-  ARBX_TRY(radix_sort_u64(ix->codes, perm.p, true, n, D * code_bits_per_axis(D), s));
+  ARBX_TRY(perm_alt.alloc((size_t)n, s));
+  unsigned long long* scodes = nullptr;   // sorted codes / permutation: whichever ping-pong buffer holds them
+  uint32_t* sperm = nullptr;
+  ARBX_TRY(radix_sort_u64(codes.p, codes_alt.p, perm.p, perm_alt.p, true, n, D * b, s, &scodes, &sperm));
 
   ARBX_TRY(scratch_alloc((void**)&ix->leaves, (size_t)n * LW * sizeof(float), s));
   const int fgrid = (int)((n + BT - 1) / BT);
   {
     ProfScope ps(K_LEAVES, s);
-    leaves_kernel<D, PK><<<fgrid, BT, 0, s>>>(prims, perm.p, n, ix->leaves);
+    leaves_kernel<D, PK><<<fgrid, BT, 0, s>>>(prims, sperm, n, ix->leaves);
     ARBX_LAUNCH_CHECK();
   }
 
@@ -375,7 +432,11 @@ arbx_status build_typed(const float* prims, int64_t n, cudaStream_t s, Index* ix
   ProfScope ps(K_HIERARCHY, s);
   constexpr int HB = HierCfg<D>::HB;
   const unsigned nchunks = (unsigned)((n + HB - 1) / HB);
-  // at most one parked subtree per distinct prefix / suffix maximum of the level bytes of a chunk
+  // A chunk parks at most one subtree per distinct prefix maximum and one per distinct suffix
+  // maximum of its level bytes.  Levels take the values 1..31 (equal codes), 33..96 (distinct
+  // codes) and 255 (array ends): at most 96 distinct values per side, 2*96 + 2 < 200.  An
+  // overflow would still not be silent: it raises BUILD_FAULT_OPEN_OVERFLOW in root[1].
+  static_assert(2 * (31 + 64 + 1) + 2 <= 200, "open_cap per chunk must cover every distinct level twice");
   const int64_t open_cap = std::min<int64_t>(n, (int64_t)nchunks * 200);
   Scratch<int> open_lrf, open_count;
   Scratch<float> open_box;
@@ -384,10 +445,10 @@ arbx_status build_typed(const float* prims, int64_t n, cudaStream_t s, Index* ix
   ARBX_TRY(open_box.alloc((size_t)open_cap * 2 * D, s));
   ARBX_CUDA(cudaMemsetAsync(open_count.p, 0, sizeof(int), s));
   ARBX_CUDA(cudaMemsetAsync(flags.p, 0xff, nn * sizeof(int), s));
-  hierarchy_kernel<D, PK><<<nchunks, HB, 0, s>>>(ix->codes, ix->leaves, ix->nodes, (int)n, ix->leaf_max, ix->root,
+  hierarchy_kernel<D, PK><<<nchunks, HB, 0, s>>>(scodes, ix->leaves, ix->nodes, (int)n, ix->leaf_max, ix->root,
                                                  open_count.p, open_lrf.p, open_box.p, (int)open_cap);
   ARBX_LAUNCH_CHECK();
-  hierarchy_top_kernel<D><<<(unsigned)((open_cap + 255) / 256), 256, 0, s>>>(ix->codes, ix->nodes, flags.p, (int)n, ix->root,
+  hierarchy_top_kernel<D><<<(unsigned)((open_cap + 255) / 256), 256, 0, s>>>(scodes, ix->nodes, flags.p, (int)n, ix->root,
                                                                            open_count.p, open_lrf.p, open_box.p, (int)open_cap);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
@@ -416,7 +477,8 @@ arbx_status build_index(const float* prims, int64_t n, int dim, int kind, cudaSt
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   ARBX_TRY(scratch_alloc((void**)&ix->bounds, 2 * ARBX_MAX_DIM * sizeof(float), s));
-  ARBX_TRY(scratch_alloc((void**)&ix->root, sizeof(int32_t), s));
+  ARBX_TRY(scratch_alloc((void**)&ix->root, 2 * sizeof(int32_t), s));
+  ARBX_CUDA(cudaMemsetAsync(ix->root, 0, 2 * sizeof(int32_t), s));
   if (n == 0) {
     empty_bounds_kernel<<<1, 32, 0, s>>>(ix->bounds, dim);
     ARBX_LAUNCH_CHECK();

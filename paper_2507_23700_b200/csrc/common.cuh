@@ -9,9 +9,12 @@
 //            idx = position in the caller's array; bit 31 set marks the LAST record of a
 //            leaf range (a collapsed subtree of <= leaf_max primitives).
 //   nodes  : one record per internal node, id = split position s (between sorted leaves s and
-//            s+1), stride 4*(D+1) floats:  lo0[D], hi0[D], lo1[D], hi1[D], c0, c1, pad, pad.
+//            s+1), stride 4*(D+1) floats:  lo0[D], hi0[D], lo1[D], hi1[D], c0, c1, l, r.
 //            A node stores the boxes of its TWO CHILDREN, so one fetch decides both descents.
 //            child ref c >= 0: internal node id; c < 0: leaf range starting at leaf ~c.
+//            [l, r] = the node's own range of sorted leaf positions (child 0 covers [l, s],
+//            child 1 covers [s+1, r]); the self-join, the packet traversals and the validator
+//            read it.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -39,12 +42,27 @@ struct Index {
   int dim = 0;
   int kind = 0;
   int leaf_max = 1;
+  int code_bits = 0;            // bits per axis of the primitive codes the tree was built from
+  bool brute = false;           // tiny index: no tree, queries scan the leaves (brute.cu)
   float* leaves = nullptr;      // n * leaf_width floats
   float* nodes = nullptr;       // max(n-1,0) * node_width floats
   float* bounds = nullptr;      // 2*dim floats: lo[dim], hi[dim] of all primitives
-  int32_t* root = nullptr;      // 1 int: root child ref (device)
-  unsigned long long* codes = nullptr;  // sorted codes, kept only for arbx_debug_validate
+  int32_t* root = nullptr;      // 2 ints (device): [0] root child ref, [1] build fault flags
 };
+constexpr int BUILD_FAULT_OPEN_OVERFLOW = 1;   // hierarchy: more parked subtrees than open_cap
+
+// Test / experiment knobs, set through arbx_debug_set (never read from the environment).
+struct DebugCfg {
+  std::atomic<int> leaf_max{16};        // primitives per collapsed leaf range
+  std::atomic<int> store_budget_mb{4096};  // scratch rows of the single-traversal storage query
+  std::atomic<int> traversal{0};        // 0 per-warp choice, 1 one query per lane, 2 packets
+  std::atomic<int> qbits{0};            // query-code bits per axis kept for the query sort (0 = all)
+  std::atomic<int> code_bits{0};        // primitive-code bits per axis (0 = adapted to n)
+  std::atomic<int> brute_max{-1};       // n <= brute_max builds a brute-force index (-1 = default)
+  std::atomic<int> l2_persist{0};       // 1: persisting-L2 window over the node array during queries
+  std::atomic<float> packet_alpha{-1.f};   // packet threshold (< 0 = default per kind / dim)
+};
+extern DebugCfg g_cfg;
 
 // ---- error plumbing ----------------------------------------------------------------------
 void set_error(const char* fmt, ...);
@@ -107,13 +125,16 @@ struct Scratch {   // RAII: released in stream order when the call returns
 };
 
 // ---- internal entry points (one per translation unit) --------------------------------------
-// sort.cu: stable LSD radix sort of bits [0,key_bits).  vals_in == nullptr means "value =
-// position" (saves writing and re-reading an iota).  Result is left in keys/vals (in place
-// from the caller's point of view; ping-pong scratch is internal).
-arbx_status radix_sort_u64(unsigned long long* keys, uint32_t* vals, bool iota_vals, int64_t n,
-                           int key_bits, cudaStream_t s);
-arbx_status radix_sort_u32(uint32_t* keys, uint32_t* vals, bool iota_vals, int64_t n,
-                           int key_bits, cudaStream_t s);
+// sort.cu: stable LSD radix sort of bits [0,key_bits) with 8-bit digits.  The caller provides
+// both ping-pong buffers; *keys_out / *vals_out tell which of them holds the result (no copy
+// back after an odd number of passes).  iota_vals: the input values are the positions 0..n-1
+// and are not read (saves writing and re-reading an iota).  vals == nullptr sorts keys only.
+arbx_status radix_sort_u64(unsigned long long* keys, unsigned long long* keys_alt, uint32_t* vals,
+                           uint32_t* vals_alt, bool iota_vals, int64_t n, int key_bits,
+                           cudaStream_t s, unsigned long long** keys_out, uint32_t** vals_out);
+arbx_status radix_sort_u32(uint32_t* keys, uint32_t* keys_alt, uint32_t* vals, uint32_t* vals_alt,
+                           bool iota_vals, int64_t n, int key_bits, cudaStream_t s,
+                           uint32_t** keys_out, uint32_t** vals_out);
 
 // build.cu
 arbx_status build_index(const float* prims, int64_t n, int dim, int kind, cudaStream_t s,
@@ -134,9 +155,13 @@ struct SpatialArgs {
   int self = 0;        // self-join: query t is the leaf at sorted position t; report later positions only
 };
 using spatial_fn = arbx_status (*)(const Index*, const SpatialArgs&, cudaStream_t);
-using knn_fn = arbx_status (*)(const Index*, const float* qpoints, int64_t nq, int k,
-                               const uint32_t* qorder, int32_t* indices, float* distances,
-                               cudaStream_t);
+// kNN: rows of k entries; kq (optional, device) gives every query its own k_q <= k, the rest of
+// its row is padding (-1 / +inf).
+struct KnnArgs {
+  const float* qpoints; int64_t nq; int k; const int32_t* kq; const uint32_t* qorder;
+  int32_t* indices; float* distances;
+};
+using knn_fn = arbx_status (*)(const Index*, const KnnArgs&, cudaStream_t);
 using qcode_fn = arbx_status (*)(const Index*, const float* queries, int64_t nq, int qkind_or_point,
                                  uint32_t* codes, int* key_bits, cudaStream_t);
 struct DimTable { spatial_fn spatial; knn_fn knn; qcode_fn qcode; };

@@ -13,6 +13,7 @@
 #include <algorithm>
 #include <cstdlib>
 #include <cstdint>
+#include <type_traits>
 
 #include "geom.cuh"
 
@@ -583,6 +584,18 @@ struct RegHeap {
       d[s - 1] = sw ? td : d[s - 1]; i[s - 1] = sw ? ti : i[s - 1];
     }
   }
+  // the same insertion as one straight compare-exchange chain: when the whole warp executes it
+  // (packet kNN) the two branches of push() would both run
+  __device__ __forceinline__ void push_uniform(float t, int32_t idx) {   // requires t < worst()
+    d[KB - 1] = t; i[KB - 1] = idx;
+#pragma unroll
+    for (int s = KB - 1; s > 0; --s) {
+      const bool sw = d[s] < d[s - 1];
+      const float td = d[s]; const int32_t ti = i[s];
+      d[s] = sw ? d[s - 1] : td; i[s] = sw ? i[s - 1] : ti;
+      d[s - 1] = sw ? td : d[s - 1]; i[s - 1] = sw ? ti : i[s - 1];
+    }
+  }
   template <class F>
   __device__ __forceinline__ void emit(int k, F&& f) {
 #pragma unroll
@@ -611,7 +624,7 @@ struct LocalHeap {
   int32_t i[ARBX_K_MAX];
   int k, m;
   __device__ __forceinline__ void init(int k_) { k = k_; m = 0; }
-  __device__ __forceinline__ float worst() const { return m < k ? INFINITY : d[0]; }
+  __device__ __forceinline__ float worst() const { return k == 0 ? -INFINITY : m < k ? INFINITY : d[0]; }
   __device__ __forceinline__ void sift_down(int pos, int size, float t, int32_t idx) {
     for (;;) {
       int c = 2 * pos + 1;
@@ -651,91 +664,298 @@ struct LocalHeap {
   }
 };
 
-// Packet kNN: the warp walks the tree once for its 32 query points.  Every lane keeps its own
-// best-k set and prunes with its own k-th distance; the warp visits a child if ANY lane still
-// needs it and takes the child that more lanes find nearer first.  Leaf-range children are
-// scanned on the spot (their size is known from the node), internal children go on the
-// shared-memory stack; a popped node is re-tested against the current bounds through its
-// children's boxes.
-template <int PK, class Heap>
-__global__ void __launch_bounds__(QT) knn_kernel(const float4* __restrict__ nodes,
-                                                 const float4* __restrict__ leaves,
-                                                 const int32_t* __restrict__ root,
-                                                 const float* __restrict__ qpoints,
-                                                 const uint32_t* __restrict__ qorder, int64_t nq, int k,
-                                                 int64_t n, int32_t* __restrict__ indices,
-                                                 float* __restrict__ distances) {
-  __shared__ int32_t s_stack[QT / 32][STACK_DEPTH];
-  int32_t* stack = s_stack[threadIdx.x >> 5];
+// ---- packet kNN (coherent warps) ---------------------------------------------------------------------
+// The 32 query points of a warp are neighbours on the curve.  When they lie close together
+// compared with their k-th neighbour distance, the warp walks the tree ONCE for all of them:
+//   1. seed bound: the warp descends from the root towards the centre c* of its query points to
+//      the smallest subtree with >= k primitives, computes the distances from c* to (at most 64
+//      of) those primitives, one or two per lane, and takes an upper bound d* of the k-th
+//      smallest of them with a 16-step radix select over ballots.  By the triangle inequality
+//      lane's k-th neighbour distance is <= d* + ||y - c*||: a VALID initial bound per lane.
+//   2. lanes-over-nodes traversal with the joint region (box J of the query points, radius
+//      Rj = largest current per-lane bound): lane i tests the two child boxes of node i of a
+//      shared-memory work list; primitives of hit leaf ranges are first filtered against
+//      (J, Rj), one primitive per lane, and only the survivors are broadcast for the exact
+//      per-lane distance and best-k insertion.  Every lane's bound shrinks to its current
+//      k-th distance as its best-k set fills, and Rj with it.
+//   3. rows are staged in shared memory and written as whole 32-byte sectors.
+// Node and leaf tests are shared by the 32 queries; what stays per lane is one exact distance
+// per surviving primitive and the insertions.  Warps that are not coherent (spread of the
+// query points > alpha * d*) are flagged and answered by knn_thread_kernel.  The joint tests
+// use the same monotone fp32 operation sequences as the exact ones, so the packet result is
+// the same set as the per-lane traversal's.
+template <int PK>
+__device__ __forceinline__ float knn_key_joint_box(const float* lo, const float* hi, const float* jlo, const float* jhi) {
+  const float d2 = dist2_bb<D>(lo, hi, jlo, jhi);
+  if constexpr (PK == KIND_SPHERE) return sqrtf(d2);
+  else return d2;
+}
+template <int PK>
+__device__ __forceinline__ float knn_key_joint_prim(const float* p, const float* jlo, const float* jhi) {
+  if constexpr (PK == KIND_POINT) return dist2_pb<D>(p, jlo, jhi);
+  else if constexpr (PK == KIND_BOX) return dist2_bb<D>(p, p + D, jlo, jhi);
+  else return fmaxf(0.f, sqrtf(dist2_pb<D>(p, jlo, jhi)) - p[D]);
+}
+
+#ifdef ARBX_STATS
+__device__ unsigned long long g_knn_stats[8];   // packet warps, fallback warps, node pops, leaf ranges, prims filtered, survivors, push rounds, lane pushes
+#define KSTAT(i, v) do { const unsigned long long v__ = (unsigned long long)(v); if (lane == 0) atomicAdd(&g_knn_stats[i], v__); } while (0)
+#else
+#define KSTAT(i, v) do { } while (0)
+#endif
+
+template <int PK, int KB>
+__global__ void __launch_bounds__(QT) knn_packet_kernel(const float4* __restrict__ nodes,
+                                                        const float4* __restrict__ leaves,
+                                                        const int32_t* __restrict__ root, int n,
+                                                        const float* __restrict__ qpoints,
+                                                        const uint32_t* __restrict__ qorder, int64_t nq,
+                                                        const int32_t* __restrict__ kq, int kmax,
+                                                        int32_t* __restrict__ indices,
+                                                        float* __restrict__ distances,
+                                                        uint8_t* __restrict__ fallback, float alpha, int force) {
+  using Heap = RegHeap<KB>;
+  constexpr int PQ_CAP = 320;                       // node work list per warp
+  constexpr int RCAP = 96;                          // candidate leaf ranges per warp (3 per lane)
+  constexpr int KBP = KB | 1;                       // odd row pitch: conflict-free staging
+  constexpr int STAGE = 32 * KBP;
+  // the node work list is dead once the leaf ranges are collected: the row staging reuses it
+  __shared__ int32_t s_work[QT / 32][(PQ_CAP > 2 * STAGE ? PQ_CAP : 2 * STAGE)];
+  __shared__ int32_t s_path[QT / 32][STACK_DEPTH];
+  __shared__ int32_t s_rfirst[QT / 32][RCAP];
+  __shared__ int32_t s_rcount[QT / 32][RCAP];
+  __shared__ float s_rdist[QT / 32][RCAP];
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int32_t* stack = s_work[w];
   const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
+  const int64_t wfirst = t - lane;
+  if (wfirst >= nq) return;
   const bool valid = t < nq;
-  const int64_t qi = valid ? (qorder ? (int64_t)qorder[t] : t) : 0;
+  // lanes past the end of the batch repeat the warp's first query: they do not change the joint region
+  const int64_t qi = qorder ? (int64_t)qorder[valid ? t : wfirst] : (valid ? t : wfirst);
   float y[D];
 #pragma unroll
   for (int a = 0; a < D; ++a) y[a] = __ldg(qpoints + qi * D + a);
+  int k = kq ? min(max(__ldg(kq + qi), 0), kmax) : kmax;
+  if (!valid) k = 0;
+  int kw = k;   // the warp's largest k: D_k is monotone in k, so its bound serves every lane
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) kw = max(kw, __shfl_xor_sync(~0u, kw, o));
+
+  // joint box of the query points and its centre
+  float jlo[D], jhi[D], cs[D];
+#pragma unroll
+  for (int a = 0; a < D; ++a) {
+    float lo = y[a], hi = y[a];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      lo = fminf(lo, __shfl_xor_sync(~0u, lo, o));
+      hi = fmaxf(hi, __shfl_xor_sync(~0u, hi, o));
+    }
+    jlo[a] = lo; jhi[a] = hi; cs[a] = 0.5f * lo + 0.5f * hi;
+  }
+  const float delta = sqrtf(dist2_pp<D>(y, cs));
+  float dmax = delta;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) dmax = fmaxf(dmax, __shfl_xor_sync(~0u, dmax, o));
+
+  // 1. seed: warp-uniform descent from the root towards c*, always into the nearer child, down to
+  // a leaf range.  The path is kept (node id, bit 30 = went into child 1) for step 2.
+  int depth = 0, smid;
+  {
+    int32_t ref = __ldg(root);
+    for (;;) {
+      NodeX nd;
+      load_node_x(nodes, ref, nd);
+      const float d0 = dist2_pb<D>(cs, nd.v, nd.v + D);
+      const float d1 = dist2_pb<D>(cs, nd.v + 2 * D, nd.v + 3 * D);
+      const bool pick1 = d1 < d0;
+      if (lane == 0) s_path[w][depth] = ref | (pick1 ? (1 << 30) : 0);
+      ++depth;
+      const int32_t child = pick1 ? nd.c1 : nd.c0;
+      if (child >= 0 && depth < STACK_DEPTH) { ref = child; continue; }
+      smid = pick1 ? (ref + 1 + nd.r) / 2 : (nd.l + ref) / 2;    // middle of the range the descent ended in
+      break;
+    }
+  }
+  __syncwarp();
+  float bound;   // per-lane initial bound in key space (squared distance; distance for SPHERE primitives)
+  {
+    // 64 consecutive sorted leaves around the end of the descent (any primitives make a valid bound)
+    const int wn = min(n, 64);
+    const int wlo = min(max(smid - wn / 2, 0), n - wn);
+    uint32_t u0 = 0x7f800000u, u1 = 0x7f800000u;
+    if (lane < wn) { Leaf<PK> lf; load_leaf<PK>(leaves, wlo + lane, lf); u0 = __float_as_uint(knn_key<PK>(cs, lf.v)); }
+    if (32 + lane < wn) { Leaf<PK> lf; load_leaf<PK>(leaves, wlo + 32 + lane, lf); u1 = __float_as_uint(knn_key<PK>(cs, lf.v)); }
+    // upper bound of the kw-th smallest key: radix select on the top 16 bits (keys are >= 0, so
+    // their bit patterns order like the values), low bits rounded up
+    uint32_t prefix = 0, mask = 0;
+    int kk = max(kw, 1);
+#pragma unroll
+    for (int bit = 30; bit >= 15; --bit) {
+      const uint32_t bb = 1u << bit;
+      const bool m0 = (u0 & mask) == prefix && !(u0 & bb);
+      const bool m1 = (u1 & mask) == prefix && !(u1 & bb);
+      const int c = __popc(__ballot_sync(~0u, m0)) + __popc(__ballot_sync(~0u, m1));
+      if (c < kk) { kk -= c; prefix |= bb; }
+      mask |= bb;
+    }
+    const float ub = __uint_as_float(prefix | 0x7fffu);
+    const float dk = PK == KIND_SPHERE ? ub : sqrtf(ub);
+    if (!force && !(dmax <= alpha * dk)) {   // not coherent: one query per lane does it
+      if (lane == 0) fallback[wfirst >> 5] = 1;
+      KSTAT(1, 1);
+      return;
+    }
+    const float b = (dk + delta) * 1.00002f;   // triangle inequality, with room for the roundings
+    bound = PK == KIND_SPHERE ? b : b * b * 1.000002f;
+  }
+  float thr = k > 0 ? bound : 0.f;            // lane inserts keys < thr = min(bound, k-th best so far)
+  float rj = thr;                             // joint radius (key space): largest thr of the warp
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) rj = fmaxf(rj, __shfl_xor_sync(~0u, rj, o));
+
+  // 2. candidate leaf ranges: everything whose box comes within rj of the joint box.  The walk
+  // starts at the highest node of the seed path whose off-path child can still matter (lane i
+  // tests level i: one round instead of one round per level of the upper tree), then runs
+  // lanes-over-nodes over a shared-memory work list.
+  int nranges = 0;
+  {
+    int start = depth - 1;
+    for (int l0 = 0; l0 < depth - 1; l0 += 32) {
+      bool rel = false;
+      if (l0 + lane < depth - 1) {
+        const int32_t e = s_path[w][l0 + lane];
+        NodeX nd;
+        load_node_x(nodes, e & ~(1 << 30), nd);
+        const bool pick1 = (e >> 30) & 1;
+        rel = (pick1 ? knn_key_joint_box<PK>(nd.v, nd.v + D, jlo, jhi)
+                     : knn_key_joint_box<PK>(nd.v + 2 * D, nd.v + 3 * D, jlo, jhi)) < rj;
+      }
+      const uint32_t m = __ballot_sync(~0u, rel);
+      if (m) { start = l0 + __ffs(m) - 1; break; }
+    }
+    const uint32_t lt = (1u << lane) - 1u;
+    int nlist = 1;
+    if (lane == 0) stack[0] = s_path[w][start] & ~(1 << 30);
+    __syncwarp();
+    while (nlist > 0) {
+      const int take = nlist > PQ_CAP - STACK_DEPTH - 64 ? 1 : min(32, nlist);
+      nlist -= take;
+      const int32_t my = lane < take ? stack[nlist + lane] : -1;
+      __syncwarp();
+      KSTAT(2, __popc(__ballot_sync(~0u, my >= 0)));
+      NodeX nd;
+      float b0 = INFINITY, b1 = INFINITY;
+      if (my >= 0) {
+        load_node_x(nodes, my, nd);
+        b0 = knn_key_joint_box<PK>(nd.v, nd.v + D, jlo, jhi);
+        b1 = knn_key_joint_box<PK>(nd.v + 2 * D, nd.v + 3 * D, jlo, jhi);
+      }
+      const bool h0 = my >= 0 && b0 < rj, h1 = my >= 0 && b1 < rj;
+      const bool lf0 = h0 && nd.c0 < 0, lf1 = h1 && nd.c1 < 0;
+      const bool in0 = h0 && nd.c0 >= 0, in1 = h1 && nd.c1 >= 0;
+      const uint32_t r0 = __ballot_sync(~0u, lf0), r1 = __ballot_sync(~0u, lf1);
+      const int nr = __popc(r0) + __popc(r1);
+      if (nranges + nr > RCAP) {               // more candidate ranges than the list holds: per-lane kernel
+        if (lane == 0) fallback[wfirst >> 5] = 1;
+        KSTAT(1, 1);
+        return;
+      }
+      if (lf0) { const int e = nranges + __popc(r0 & lt); s_rfirst[w][e] = nd.l; s_rcount[w][e] = my - nd.l + 1; s_rdist[w][e] = b0; }
+      if (lf1) { const int e = nranges + __popc(r0) + __popc(r1 & lt); s_rfirst[w][e] = my + 1; s_rcount[w][e] = nd.r - my; s_rdist[w][e] = b1; }
+      nranges += nr;
+      const uint32_t q0 = __ballot_sync(~0u, in0), q1 = __ballot_sync(~0u, in1);
+      if (in0) stack[nlist + __popc(q0 & lt)] = nd.c0;
+      if (in1) stack[nlist + __popc(q0) + __popc(q1 & lt)] = nd.c1;
+      nlist += __popc(q0) + __popc(q1);
+      __syncwarp();
+    }
+  }
+  KSTAT(0, 1);
+
+  // 3. the ranges nearest-first; every lane's bound shrinks to its current k-th distance as its
+  // best-k set fills, the joint radius with it, and the walk ends when the nearest unvisited
+  // range lies beyond the joint radius
   Heap heap;
   heap.init(k);
-
-  auto leaf_range = [&](int first, int m) {   // m is warp-uniform
-    constexpr int CH = 4;   // the loads and keys of a chunk are independent of its pushes
-    for (int j0 = 0; j0 < m; j0 += CH) {
-      float key[CH];
-      int32_t id[CH];
+  {
+    float rd[RCAP / 32];
 #pragma unroll
-      for (int j = 0; j < CH; ++j) {
-        Leaf<PK> lf;
-        load_leaf<PK>(leaves, min(first + j0 + j, first + m - 1), lf);
-        key[j] = j0 + j < m ? knn_key<PK>(y, lf.v) : INFINITY;
-        id[j] = (int32_t)(lf.idx & ~LEAF_END);
+    for (int j = 0; j < RCAP / 32; ++j) rd[j] = j * 32 + lane < nranges ? s_rdist[w][j * 32 + lane] : INFINITY;
+    for (;;) {
+      float best = rd[0];
+      int bi = lane;
+#pragma unroll
+      for (int j = 1; j < RCAP / 32; ++j)
+        if (rd[j] < best) { best = rd[j]; bi = j * 32 + lane; }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        const float ob = __shfl_xor_sync(~0u, best, o);
+        const int oi = __shfl_xor_sync(~0u, bi, o);
+        if (ob < best || (ob == best && oi < bi)) { best = ob; bi = oi; }
       }
+      if (!(best < rj)) break;
 #pragma unroll
-      for (int j = 0; j < CH; ++j)
-        if (valid && key[j] < heap.worst()) heap.push(key[j], id[j]);
+      for (int j = 0; j < RCAP / 32; ++j)
+        if (bi == j * 32 + lane) rd[j] = INFINITY;
+      const int first = s_rfirst[w][bi], m = s_rcount[w][bi];
+      KSTAT(3, 1); KSTAT(4, m);
+      for (int j0 = 0; j0 < m; j0 += 32) {
+        bool in = false;
+        if (j0 + lane < m) {
+          Leaf<PK> mine;
+          load_leaf<PK>(leaves, first + j0 + lane, mine);
+          in = knn_key_joint_prim<PK>(mine.v, jlo, jhi) < rj;
+        }
+        uint32_t todo = __ballot_sync(~0u, in);
+        KSTAT(5, __popc(todo));
+        while (todo) {
+          const int b = __ffs(todo) - 1;
+          todo &= todo - 1;
+          Leaf<PK> lf;
+          load_leaf<PK>(leaves, first + j0 + b, lf);
+          const float key = knn_key<PK>(y, lf.v);
+#ifdef ARBX_STATS
+          { const uint32_t pm = __ballot_sync(~0u, key < thr); KSTAT(6, pm != 0); KSTAT(7, __popc(pm)); }
+#endif
+          if (key < thr) {
+            heap.push_uniform(key, (int32_t)(lf.idx & ~LEAF_END));
+            thr = fminf(thr, heap.worst());
+          }
+        }
+      }
+      rj = thr;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) rj = fmaxf(rj, __shfl_xor_sync(~0u, rj, o));
+    }
+  }
+
+  // 4. emit: stage the rows, then write them as runs of whole sectors
+  __syncwarp();
+  float* sd = reinterpret_cast<float*>(s_work[w]);
+  int32_t* si = s_work[w] + STAGE;
+  heap.emit(k, [&](int pos, float key, int32_t idx) {
+    sd[lane * KBP + pos] = (PK == KIND_SPHERE || idx < 0) ? key : sqrtf(key);
+    si[lane * KBP + pos] = idx;
+  });
+  for (int pos = k; pos < kmax; ++pos) { sd[lane * KBP + pos] = INFINITY; si[lane * KBP + pos] = -1; }
+  __syncwarp();
+  const int total = (int)min((int64_t)32, nq - wfirst) * kmax;
+  auto write_rows = [&](auto kconst) {            // kconst: compile-time row length, or 0 for kmax
+    const int kk = decltype(kconst)::value ? decltype(kconst)::value : kmax;
+    for (int e0 = 0; e0 < total; e0 += 32) {      // warp-uniform trip count: the shuffle needs every lane
+      const int e = min(e0 + lane, total - 1);
+      const int row = e / kk, slot = e - row * kk;
+      const int64_t q = __shfl_sync(~0u, qi, row);
+      if (e0 + lane < total) {
+        indices[q * kk + slot] = si[row * KBP + slot];
+        if (distances) distances[q * kk + slot] = sd[row * KBP + slot];
+      }
     }
   };
-
-  if (n > 0) {
-    int32_t ref = __ldg(root);
-    if (ref < 0) {
-      leaf_range(0, (int)n);
-    } else {
-      int sp = 0;
-      for (;;) {
-        NodeX nd;
-        load_node_x(nodes, ref, nd);
-        const float b0 = knn_bound<PK>(y, nd.v, nd.v + D);
-        const float b1 = knn_bound<PK>(y, nd.v + 2 * D, nd.v + 3 * D);
-        // child 1 first if more lanes find it nearer
-        const bool swap = __popc(__ballot_sync(~0u, valid && b1 < b0)) > __popc(__ballot_sync(~0u, valid && b0 < b1));
-        const float bn = swap ? b1 : b0, bf = swap ? b0 : b1;
-        const int32_t cn = swap ? nd.c1 : nd.c0, cf = swap ? nd.c0 : nd.c1;
-        int32_t next = -1;
-        if (__any_sync(~0u, valid && bn < heap.worst())) {
-          if (cn < 0) { if (swap) leaf_range(ref + 1, nd.r - ref); else leaf_range(nd.l, ref - nd.l + 1); }
-          else next = cn;
-        }
-        if (__any_sync(~0u, valid && bf < heap.worst())) {
-          if (cf < 0) { if (swap) leaf_range(nd.l, ref - nd.l + 1); else leaf_range(ref + 1, nd.r - ref); }
-          else if (next >= 0) stack[sp++] = cf;
-          else next = cf;
-        }
-        if (next >= 0) { ref = next; continue; }
-        if (sp == 0) break;
-        ref = stack[--sp];
-      }
-    }
-  }
-  if (!valid) return;
-  int32_t* oi = indices + qi * k;
-  float* od = distances ? distances + qi * k : nullptr;
-  if constexpr (Heap::kVec) {
-    // sqrt(+inf) = +inf keeps the padding of short rows (n < k) intact
-    if (k == Heap::kSlots) { heap.emit_vec(oi, od, PK != KIND_SPHERE); return; }
-  }
-  heap.emit(k, [&](int s, float key, int32_t idx) {
-    oi[s] = idx;
-    if (od) od[s] = (PK == KIND_SPHERE || idx < 0) ? key : sqrtf(key);
-  });
+  if (kmax == KB) write_rows(std::integral_constant<int, KB>{});
+  else write_rows(std::integral_constant<int, 0>{});
 }
 
 // ---- one query per thread (independent traversal) --------------------------------------------------
@@ -747,15 +967,19 @@ __global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict
                                                  const float4* __restrict__ leaves,
                                                  const int32_t* __restrict__ root,
                                                  const float* __restrict__ qpoints,
-                                                 const uint32_t* __restrict__ qorder, int64_t nq, int k,
+                                                 const uint32_t* __restrict__ qorder, int64_t nq,
+                                                 const int32_t* __restrict__ kq, int kmax,
                                                  int64_t n, int32_t* __restrict__ indices,
-                                                 float* __restrict__ distances) {
+                                                 float* __restrict__ distances,
+                                                 const uint8_t* __restrict__ only, int vec_ok) {
   const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
   if (t >= nq) return;
+  if (only && !only[t >> 5]) return;   // this warp was answered by the packet kernel
   const int64_t qi = qorder ? (int64_t)qorder[t] : t;
   float y[D];
 #pragma unroll
   for (int a = 0; a < D; ++a) y[a] = __ldg(qpoints + qi * D + a);
+  const int k = kq ? min(max(__ldg(kq + qi), 0), kmax) : kmax;
   Heap heap;
   heap.init(k);
   if (n > 0) {
@@ -802,24 +1026,24 @@ __global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict
       ref = pop();
     }
   }
-  int32_t* oi = indices + qi * k;
-  float* od = distances ? distances + qi * k : nullptr;
+  int32_t* oi = indices + qi * kmax;
+  float* od = distances ? distances + qi * kmax : nullptr;
   if constexpr (Heap::kVec) {
-    // sqrt(+inf) = +inf keeps the padding of short rows (n < k) intact
-    if (k == Heap::kSlots) { heap.emit_vec(oi, od, PK != KIND_SPHERE); return; }
+    // rows of exactly kSlots entries on 16-byte aligned outputs: 128-bit stores
+    // (sqrt(+inf) = +inf keeps the padding of short rows (n < k) intact)
+    if (vec_ok && k == Heap::kSlots) { heap.emit_vec(oi, od, PK != KIND_SPHERE); return; }
   }
   heap.emit(k, [&](int s, float key, int32_t idx) {
     oi[s] = idx;
     if (od) od[s] = (PK == KIND_SPHERE || idx < 0) ? key : sqrtf(key);
   });
+  for (int s = k; s < kmax; ++s) {      // per-query k: the rest of the row is padding
+    oi[s] = -1;
+    if (od) od[s] = INFINITY;
+  }
 }
 
-// Experiment switch ARBX_TRAVERSAL: unset = default (packet spatial, per-thread kNN),
-// "thread" = one query per thread everywhere, "packet" = packets everywhere.
-inline int traversal_mode() {
-  const char* v = getenv("ARBX_TRAVERSAL");
-  return !v ? 0 : v[0] == 't' ? 1 : v[0] == 'p' ? 2 : 0;
-}
+inline int traversal_mode() { return g_cfg.traversal.load(std::memory_order_relaxed); }
 
 // ---- host dispatch ------------------------------------------------------------------------------------
 template <int PK, int QK, bool SELF = false>
@@ -832,7 +1056,7 @@ arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s
   // packet threshold (spread of the warp's query centres <= alpha * query extent), measured:
   // 1.5 (spheres) / 2.5 (boxes) up to 3-D, 0.75 above (the joint region gets loose quickly)
   float alpha = D <= 3 ? (QK == KIND_BOX ? 2.5f : 1.5f) : 0.75f;
-  if (const char* v = getenv("ARBX_PACKET_ALPHA")) alpha = (float)atof(v);
+  if (const float v = g_cfg.packet_alpha.load(std::memory_order_relaxed); v >= 0.f) alpha = v;
   const int n = (int)ix->n;
   if (a.pass == 1)
     spatial_kernel<PK, QK, 1, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, a.stop_fill, mode, alpha);
@@ -866,40 +1090,59 @@ arbx_status spatial_entry(const Index* ix, const SpatialArgs& a, cudaStream_t s)
 }
 
 template <int PK, class Heap>
-arbx_status knn_launch(const Index* ix, const float* qpoints, int64_t nq, int k, const uint32_t* qorder,
-                       int32_t* indices, float* distances, cudaStream_t s) {
-  const unsigned grid = (unsigned)((nq + QT - 1) / QT);
-  ProfScope ps(K_KNN, s);
-  if (traversal_mode() == 2)
-    knn_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
-                                             reinterpret_cast<const float4*>(ix->leaves), ix->root, qpoints,
-                                             qorder, nq, k, ix->n, indices, distances);
-  else
-    knn_thread_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
-                                                    reinterpret_cast<const float4*>(ix->leaves), ix->root, qpoints,
-                                                    qorder, nq, k, ix->n, indices, distances);
+arbx_status knn_thread_launch(const Index* ix, const KnnArgs& a, const uint8_t* only, cudaStream_t s) {
+  const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);
+  // 128-bit row stores need 16-byte aligned output pointers (rows of 4, 8, 16, 32 entries then stay aligned)
+  const int vec_ok = !a.kq && ((reinterpret_cast<uintptr_t>(a.indices) | reinterpret_cast<uintptr_t>(a.distances)) & 15) == 0;
+  knn_thread_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
+                                                  reinterpret_cast<const float4*>(ix->leaves), ix->root, a.qpoints,
+                                                  a.qorder, a.nq, a.kq, a.k, ix->n, a.indices, a.distances, only, vec_ok);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
 
-template <int PK>
-arbx_status knn_pk(const Index* ix, const float* qpoints, int64_t nq, int k, const uint32_t* qorder,
-                   int32_t* indices, float* distances, cudaStream_t s) {
-  if (k <= 1) return knn_launch<PK, RegHeap<1>>(ix, qpoints, nq, k, qorder, indices, distances, s);
-  if (k <= 2) return knn_launch<PK, RegHeap<2>>(ix, qpoints, nq, k, qorder, indices, distances, s);
-  if (k <= 4) return knn_launch<PK, RegHeap<4>>(ix, qpoints, nq, k, qorder, indices, distances, s);
-  if (k <= 8) return knn_launch<PK, RegHeap<8>>(ix, qpoints, nq, k, qorder, indices, distances, s);
-  if (k <= 16) return knn_launch<PK, RegHeap<16>>(ix, qpoints, nq, k, qorder, indices, distances, s);
-  if (k <= 32) return knn_launch<PK, RegHeap<32>>(ix, qpoints, nq, k, qorder, indices, distances, s);
-  return knn_launch<PK, LocalHeap>(ix, qpoints, nq, k, qorder, indices, distances, s);
+// Packet kernel for the coherent warps, per-lane kernel for the rest (flagged per warp).
+template <int PK, int KB>
+arbx_status knn_launch(const Index* ix, const KnnArgs& a, cudaStream_t s) {
+  ProfScope ps(K_KNN, s);
+  const int mode = traversal_mode();
+  // the packet path needs a real tree and a seed subtree of >= k primitives
+  const bool packet = mode != 1 && ix->n >= 4 * (int64_t)a.k && ix->n > 4 * (int64_t)ix->leaf_max && ix->n >= 64;
+  if (!packet) return knn_thread_launch<PK, RegHeap<KB>>(ix, a, nullptr, s);
+  const int64_t nwarps = (a.nq + 31) / 32;
+  Scratch<uint8_t> flags;
+  ARBX_TRY(flags.alloc((size_t)nwarps, s));
+  ARBX_CUDA(cudaMemsetAsync(flags.p, 0, (size_t)nwarps, s));
+  float alpha = D <= 3 ? 1.0f : 0.5f;
+  if (const float v = g_cfg.packet_alpha.load(std::memory_order_relaxed); v >= 0.f) alpha = v;
+  const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);
+  knn_packet_kernel<PK, KB><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
+                                                reinterpret_cast<const float4*>(ix->leaves), ix->root, (int)ix->n,
+                                                a.qpoints, a.qorder, a.nq, a.kq, a.k, a.indices, a.distances,
+                                                flags.p, alpha, mode == 2 ? 1 : 0);
+  ARBX_LAUNCH_CHECK();
+  // (forced packets still leave the warps with too many candidate ranges to the per-lane kernel)
+  return knn_thread_launch<PK, RegHeap<KB>>(ix, a, flags.p, s);
 }
 
-arbx_status knn_entry(const Index* ix, const float* qpoints, int64_t nq, int k, const uint32_t* qorder,
-                      int32_t* indices, float* distances, cudaStream_t s) {
+template <int PK>
+arbx_status knn_pk(const Index* ix, const KnnArgs& a, cudaStream_t s) {
+  const int k = a.k;
+  if (k <= 1) return knn_launch<PK, 1>(ix, a, s);
+  if (k <= 2) return knn_launch<PK, 2>(ix, a, s);
+  if (k <= 4) return knn_launch<PK, 4>(ix, a, s);
+  if (k <= 8) return knn_launch<PK, 8>(ix, a, s);
+  if (k <= 16) return knn_launch<PK, 16>(ix, a, s);
+  if (k <= 32) return knn_launch<PK, 32>(ix, a, s);
+  ProfScope ps(K_KNN, s);
+  return knn_thread_launch<PK, LocalHeap>(ix, a, nullptr, s);
+}
+
+arbx_status knn_entry(const Index* ix, const KnnArgs& a, cudaStream_t s) {
   switch (ix->kind) {
-    case KIND_POINT: return knn_pk<KIND_POINT>(ix, qpoints, nq, k, qorder, indices, distances, s);
-    case KIND_BOX: return knn_pk<KIND_BOX>(ix, qpoints, nq, k, qorder, indices, distances, s);
-    default: return knn_pk<KIND_SPHERE>(ix, qpoints, nq, k, qorder, indices, distances, s);
+    case KIND_POINT: return knn_pk<KIND_POINT>(ix, a, s);
+    case KIND_BOX: return knn_pk<KIND_BOX>(ix, a, s);
+    default: return knn_pk<KIND_SPHERE>(ix, a, s);
   }
 }
 
@@ -913,7 +1156,7 @@ arbx_status qcode_entry(const Index* ix, const float* queries, int64_t nq, int q
   // the sort key keeps the top `qb` bits per axis of the code (whole 8-bit digit passes)
   constexpr int B = qcode_bits_per_axis(D);
   int qb = B;
-  if (const char* v = getenv("ARBX_QBITS")) qb = std::max(1, std::min(B, atoi(v)));
+  if (const int v = g_cfg.qbits.load(std::memory_order_relaxed); v > 0) qb = std::max(1, std::min(B, v));
   const int drop = D * (B - qb);
   switch (qkind) {
     case KIND_POINT: qcode_kernel<KIND_POINT><<<grid, 256, 0, s>>>(queries, nq, ix->bounds, codes, drop); break;
@@ -924,6 +1167,17 @@ arbx_status qcode_entry(const Index* ix, const float* queries, int64_t nq, int q
   *key_bits = D * qb;
   return ARBX_OK;
 }
+
+#ifdef ARBX_STATS
+}  // namespace
+void knn_stats_read(unsigned long long* out) {   // debug builds only (-DARBX_STATS, dimension ARBX_DIM)
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, g_knn_stats, sizeof(g_knn_stats));
+  unsigned long long z[8] = {};
+  cudaMemcpyToSymbol(g_knn_stats, z, sizeof(z));
+}
+namespace {
+#endif
 
 const DimTable kTable = {spatial_entry, knn_entry, qcode_entry};
 

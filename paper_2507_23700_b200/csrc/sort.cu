@@ -8,6 +8,8 @@
 //
 // Algorithmic HBM bytes per element: histogram K; per pass 2*(K+4)
 // (K = key bytes; the first pass of an iota sort reads no values).
+#include <atomic>
+
 #include "common.cuh"
 
 namespace arbx {
@@ -49,7 +51,9 @@ __device__ __forceinline__ uint32_t match_digit(uint32_t d) {
 // ---- histogram of every digit in one read of the keys ---------------------------------------
 template <typename K>
 __global__ void __launch_bounds__(512) hist_kernel(const K* __restrict__ keys, uint32_t n, int npass,
-                                                   uint32_t* __restrict__ ghist) {
+                                                   uint32_t top_mask, uint32_t* __restrict__ ghist) {
+  // top_mask: bits of the last digit that belong to the key (bits at or above key_bits are ignored)
+  auto digit = [&](K k, int p) -> uint32_t { return (uint32_t)(k >> (8 * p)) & (p == npass - 1 ? top_mask : 255u); };
   __shared__ uint32_t sh[MAX_PASSES * RADIX];
   for (int i = threadIdx.x; i < npass * RADIX; i += blockDim.x) sh[i] = 0;
   __syncthreads();
@@ -67,12 +71,12 @@ __global__ void __launch_bounds__(512) hist_kernel(const K* __restrict__ keys, u
     }
 #pragma unroll
     for (int e = 0; e < VEC; ++e)
-      for (int p = 0; p < npass; ++p) atomicAdd(&sh[p * RADIX + (uint32_t)((k[e] >> (8 * p)) & 255)], 1u);
+      for (int p = 0; p < npass; ++p) atomicAdd(&sh[p * RADIX + digit(k[e], p)], 1u);
   }
   if (blockIdx.x == 0) {
     for (uint32_t i = nvec * VEC + threadIdx.x; i < n; i += blockDim.x) {
       K k = keys[i];
-      for (int p = 0; p < npass; ++p) atomicAdd(&sh[p * RADIX + (uint32_t)((k >> (8 * p)) & 255)], 1u);
+      for (int p = 0; p < npass; ++p) atomicAdd(&sh[p * RADIX + digit(k, p)], 1u);
     }
   }
   __syncthreads();
@@ -102,7 +106,7 @@ __global__ void __launch_bounds__(RADIX) hist_scan_kernel(uint32_t* ghist) {
 template <typename K, bool IOTA, bool VALS>
 __global__ void __launch_bounds__(SORT_THREADS, 2)
 onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* __restrict__ vin,
-              uint32_t* __restrict__ vout, uint32_t n, int shift,
+              uint32_t* __restrict__ vout, uint32_t n, int shift, uint32_t dmask,
               const uint32_t* __restrict__ digit_base, uint32_t* __restrict__ counter,
               uint32_t* __restrict__ status) {
   // dynamic shared memory: the tile (keys, later reused for values) then the per-warp digit counters
@@ -123,14 +127,16 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
   const uint32_t tile_base = tile * (uint32_t)SORT_TILE;
   const uint32_t nvalid = min((uint32_t)SORT_TILE, n - tile_base);
 
-  // warp-striped load: warp w owns SORT_IPT*32 consecutive elements
+  // warp-striped load: warp w owns SORT_IPT*32 consecutive elements.  Padding keys of a partial
+  // last tile carry the largest digit of this pass, so they sort behind every real key.
   K key[SORT_IPT];
   uint32_t val[SORT_IPT];
   const uint32_t wbase = tile_base + w * (32 * SORT_IPT) + lane;
+  const K pad_key = (K)dmask << shift;
 #pragma unroll
   for (int j = 0; j < SORT_IPT; ++j) {
     uint32_t idx = wbase + j * 32;
-    key[j] = idx < n ? kin[idx] : (K)~(K)0;
+    key[j] = idx < n ? kin[idx] : pad_key;
     if constexpr (VALS) val[j] = IOTA ? idx : (idx < n ? vin[idx] : 0u);
   }
 
@@ -146,10 +152,10 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
     uint32_t peers[MB];
 #pragma unroll
     for (int j = 0; j < MB; ++j)
-      peers[j] = match_digit((uint32_t)(key[j0 + j] >> shift) & 255u);
+      peers[j] = match_digit((uint32_t)(key[j0 + j] >> shift) & dmask);
 #pragma unroll
     for (int j = 0; j < MB; ++j) {
-      const uint32_t d = (uint32_t)(key[j0 + j] >> shift) & 255u;
+      const uint32_t d = (uint32_t)(key[j0 + j] >> shift) & dmask;
       const int leader = __ffs(peers[j]) - 1;
       uint32_t old = 0;
       if (lane == leader) old = atomicAdd(&whist[w][d], (uint32_t)__popc(peers[j]));
@@ -169,9 +175,9 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
       whist[i][d] = run;
       run += t;
     }
-    // padding keys (all ones) of a partial last tile sit in digit 255; nobody reads their count
+    // padding keys of a partial last tile sit in digit dmask; nobody reads their count
     pub = run;
-    if (d == 255) pub -= (uint32_t)SORT_TILE - nvalid;
+    if (d == (int)dmask) pub -= (uint32_t)SORT_TILE - nvalid;
     st_volatile_u32(&status[(size_t)tile * RADIX + d], (tile == 0 ? FLAG_INCL : FLAG_AGG) | pub);
 
     // exclusive scan of the tile counts over digits
@@ -227,7 +233,7 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
   uint16_t pos[SORT_IPT];
 #pragma unroll
   for (int j = 0; j < SORT_IPT; ++j) {
-    const uint32_t d = (uint32_t)(key[j] >> shift) & 255u;
+    const uint32_t d = (uint32_t)(key[j] >> shift) & dmask;
     pos[j] = (uint16_t)(s_toff[d] + whist[w][d] + rank[j]);
     sm.keys[pos[j]] = key[j];
   }
@@ -237,7 +243,7 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
   for (int j = 0; j < SORT_IPT; ++j) {
     const uint32_t p = j * SORT_THREADS + tid;
     const K k = sm.keys[p];
-    const uint32_t d = (uint32_t)(k >> shift) & 255u;
+    const uint32_t d = (uint32_t)(k >> shift) & dmask;
     gpos[j] = s_goff[d] + p;
     if (p < nvalid) kout[gpos[j]] = k;
   }
@@ -255,7 +261,10 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
 }
 
 template <typename K>
-arbx_status radix_sort_impl(K* keys, uint32_t* vals, bool iota, int64_t n, int key_bits, cudaStream_t s) {
+arbx_status radix_sort_impl(K* keys, K* kalt, uint32_t* vals, uint32_t* valt, bool iota, int64_t n, int key_bits,
+                            cudaStream_t s, K** keys_out, uint32_t** vals_out) {
+  *keys_out = keys;
+  *vals_out = vals;
   if (n <= 0) return ARBX_OK;
   if (n > (int64_t(1) << 30)) { set_error("radix sort: n > 2^30"); return ARBX_ERR_UNSUPPORTED; }
   const bool has_vals = vals != nullptr;
@@ -263,15 +272,13 @@ arbx_status radix_sort_impl(K* keys, uint32_t* vals, bool iota, int64_t n, int k
     if (has_vals && iota) { ARBX_CUDA(cudaMemsetAsync(vals, 0, sizeof(uint32_t), s)); }
     return ARBX_OK;
   }
-  int npass = (key_bits + 7) / 8;
-  if (npass < 1) npass = 1;
-  if (npass > (int)sizeof(K)) npass = (int)sizeof(K);
+  if (key_bits < 1) key_bits = 1;
+  if (key_bits > 8 * (int)sizeof(K)) key_bits = 8 * (int)sizeof(K);
+  const int npass = (key_bits + 7) / 8;
+  const uint32_t top_mask = key_bits % 8 ? (1u << (key_bits % 8)) - 1u : 255u;
   const uint32_t ntiles = (uint32_t)((n + SORT_TILE - 1) / SORT_TILE);
 
-  Scratch<K> kalt;
-  Scratch<uint32_t> valt, meta;
-  ARBX_TRY(kalt.alloc((size_t)n, s));
-  if (has_vals) ARBX_TRY(valt.alloc((size_t)n, s));
+  Scratch<uint32_t> meta;
   // meta: [npass*256] digit histograms | [npass] tile counters | [npass*ntiles*256] look-back status
   const size_t meta_words = (size_t)npass * RADIX + MAX_PASSES + (size_t)npass * ntiles * RADIX;
   ARBX_TRY(meta.alloc(meta_words, s));
@@ -289,47 +296,52 @@ arbx_status radix_sort_impl(K* keys, uint32_t* vals, bool iota, int64_t n, int k
     ProfScope ps(kHistId, s);
     int64_t want = (n / (16 / (int)sizeof(K)) + 511) / 512;
     int grid = (int)std::min<int64_t>(std::max<int64_t>(want, 1), (int64_t)sms * 4);
-    hist_kernel<K><<<grid, 512, 0, s>>>(keys, (uint32_t)n, npass, ghist);
+    hist_kernel<K><<<grid, 512, 0, s>>>(keys, (uint32_t)n, npass, top_mask, ghist);
     ARBX_LAUNCH_CHECK();
     hist_scan_kernel<<<npass, RADIX, 0, s>>>(ghist);
     ARBX_LAUNCH_CHECK();
   }
   const size_t smem = (sizeof(K) > 4 ? sizeof(K) : 4) * SORT_TILE + sizeof(uint32_t) * SORT_WARPS * RADIX;
-  ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  K* kin = keys; K* kout = kalt.p;
-  uint32_t* vin = vals; uint32_t* vout = valt.p;
+  static std::atomic<bool> attr_set{false};   // one instance per key type K
+  if (!attr_set.load(std::memory_order_acquire)) {
+    ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set.store(true, std::memory_order_release);
+  }
+  K* kin = keys; K* kout = kalt;
+  uint32_t* vin = vals; uint32_t* vout = valt;
   for (int p = 0; p < npass; ++p) {
     const uint32_t* base = ghist + (size_t)p * RADIX;
     uint32_t* st = status + (size_t)p * ntiles * RADIX;
+    const uint32_t dmask = p == npass - 1 ? top_mask : 255u;
     ProfScope ps(kPassId, s);
     if (!has_vals)
-      onesweep_pass<K, false, false><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, nullptr, nullptr, (uint32_t)n, 8 * p, base, counters + p, st);
+      onesweep_pass<K, false, false><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, nullptr, nullptr, (uint32_t)n, 8 * p, dmask, base, counters + p, st);
     else if (p == 0 && iota)
-      onesweep_pass<K, true, true><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, nullptr, vout, (uint32_t)n, 8 * p, base, counters + p, st);
+      onesweep_pass<K, true, true><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, nullptr, vout, (uint32_t)n, 8 * p, dmask, base, counters + p, st);
     else
-      onesweep_pass<K, false, true><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, vin, vout, (uint32_t)n, 8 * p, base, counters + p, st);
+      onesweep_pass<K, false, true><<<ntiles, SORT_THREADS, smem, s>>>(kin, kout, vin, vout, (uint32_t)n, 8 * p, dmask, base, counters + p, st);
     ARBX_LAUNCH_CHECK();
     std::swap(kin, kout);
     std::swap(vin, vout);
   }
-  if (kin != keys) {   // odd number of passes: result sits in the scratch buffers
-    ARBX_CUDA(cudaMemcpyAsync(keys, kin, (size_t)n * sizeof(K), cudaMemcpyDeviceToDevice, s));
-    if (has_vals) ARBX_CUDA(cudaMemcpyAsync(vals, vin, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, s));
-  }
+  *keys_out = kin;
+  *vals_out = vin;
   return ARBX_OK;
 }
 
 }  // namespace
 
-arbx_status radix_sort_u64(unsigned long long* keys, uint32_t* vals, bool iota_vals, int64_t n,
-                           int key_bits, cudaStream_t s) {
-  return radix_sort_impl<unsigned long long>(keys, vals, iota_vals, n, key_bits, s);
+arbx_status radix_sort_u64(unsigned long long* keys, unsigned long long* keys_alt, uint32_t* vals,
+                           uint32_t* vals_alt, bool iota_vals, int64_t n, int key_bits,
+                           cudaStream_t s, unsigned long long** keys_out, uint32_t** vals_out) {
+  return radix_sort_impl<unsigned long long>(keys, keys_alt, vals, vals_alt, iota_vals, n, key_bits, s, keys_out, vals_out);
 }
-arbx_status radix_sort_u32(uint32_t* keys, uint32_t* vals, bool iota_vals, int64_t n, int key_bits,
-                           cudaStream_t s) {
-  return radix_sort_impl<uint32_t>(keys, vals, iota_vals, n, key_bits, s);
+arbx_status radix_sort_u32(uint32_t* keys, uint32_t* keys_alt, uint32_t* vals, uint32_t* vals_alt,
+                           bool iota_vals, int64_t n, int key_bits, cudaStream_t s,
+                           uint32_t** keys_out, uint32_t** vals_out) {
+  return radix_sort_impl<uint32_t>(keys, keys_alt, vals, vals_alt, iota_vals, n, key_bits, s, keys_out, vals_out);
 }
 
 }  // namespace arbx

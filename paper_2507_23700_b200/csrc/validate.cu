@@ -1,6 +1,7 @@
 // validate.cu -- structural self-check of the tree (test hook, SURVEY.md §8(c-5) pin P9).
 // Not on the hot path.  Checks, on the device:
-//   V1 sorted codes are non-decreasing;
+//   V0 the build raised no fault flag;
+//   V1 the codes of the leaves (recomputed from the leaf records) are non-decreasing;
 //   V2 the leaf indices are a permutation of [0,n);
 //   V3 every real internal node (range larger than leaf_max) has children whose ranges
 //      partition its own range at its split position, and each stored child box equals the
@@ -14,9 +15,32 @@ namespace {
 
 __device__ __forceinline__ void fail(unsigned long long* v) { atomicAdd(v, 1ull); }
 
-__global__ void v_codes_kernel(const unsigned long long* codes, int n, unsigned long long* viol) {
+// V1: the codes are not kept after the build; they are recomputed here from the leaf records
+// (the same geometry, the same quantisation) and must be non-decreasing along the leaves.
+template <int D, int PK>
+__device__ unsigned long long leaf_code(const float* leaves, int j, const float* bounds, int drop) {
+  constexpr int W = prim_width(PK, D);
+  constexpr int LW = leaf_width(PK, D);
+  constexpr int B = code_bits_per_axis(D);
+  float v[W], c[D], lo[D], scale[D];
+  for (int e = 0; e < W; ++e) v[e] = leaves[(int64_t)j * LW + e];
+  for (int a = 0; a < D; ++a) {
+    lo[a] = bounds[a];
+    const float ext = bounds[D + a] - lo[a];
+    scale[a] = ext > 0.f ? exp2f((float)B) / ext : 0.f;
+  }
+  centre_of<D, PK>(v, c);
+  uint32_t q[D];
+  quantise<D, B>(c, lo, scale, q);
+  return interleave<D, B, unsigned long long>(q) >> drop;
+}
+template <int D, int PK>
+__global__ void v_codes_kernel(const float* leaves, const float* bounds, int n, int drop, unsigned long long* viol) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i + 1 < n && codes[i] > codes[i + 1]) fail(viol);
+  if (i + 1 < n && leaf_code<D, PK>(leaves, i, bounds, drop) > leaf_code<D, PK>(leaves, i + 1, bounds, drop)) fail(viol);
+}
+__global__ void v_fault_kernel(const int32_t* root, unsigned long long* viol) {
+  if (root[1] != 0) fail(viol);   // V0: the build raised a fault flag (parked-subtree list overflow)
 }
 
 __global__ void v_perm_kernel(const float* leaves, int LW, int W, int n, int* seen,
@@ -142,7 +166,8 @@ arbx_status validate_typed(const Index* ix, unsigned long long* viol, cudaStream
   ARBX_CUDA(cudaMemsetAsync(cover.p, 0, sizeof(int) * n, s));
   ARBX_CUDA(cudaMemsetAsync(refcnt.p, 0, sizeof(int) * n, s));
   ARBX_CUDA(cudaMemsetAsync(real.p, 0, sizeof(int) * n, s));
-  v_codes_kernel<<<g, T, 0, s>>>(ix->codes, n, viol); ARBX_LAUNCH_CHECK();
+  v_fault_kernel<<<1, 1, 0, s>>>(ix->root, viol); ARBX_LAUNCH_CHECK();
+  if (!ix->brute) v_codes_kernel<D, PK><<<g, T, 0, s>>>(ix->leaves, ix->bounds, n, D * (code_bits_per_axis(D) - ix->code_bits), viol); ARBX_LAUNCH_CHECK();
   v_perm_kernel<<<g, T, 0, s>>>(ix->leaves, leaf_width(PK, D), prim_width(PK, D), n, seen.p, viol); ARBX_LAUNCH_CHECK();
   v_ones_kernel<<<g, T, 0, s>>>(seen.p, n, viol); ARBX_LAUNCH_CHECK();
   if (n > 1) { v_nodes_kernel<D, PK><<<g, T, 0, s>>>(ix->leaves, ix->nodes, n, ix->leaf_max, refcnt.p, cover.p, real.p, viol); ARBX_LAUNCH_CHECK(); }

@@ -18,10 +18,19 @@ def test_algorithmic_bytes_match_survey_table():
     n = cfg["n"]
     assert b["B1_bounds"] == 12 * n                                   # 12 B/prim
     assert b["B2_codes"] == 20 * n
-    assert b["B3_sort_hist"] + b["B3_sort_pass"] == (8 + 20 + 7 * 24) * n
+    assert bench.sort_passes(n, 3) == 5                               # 13 bits per axis at N = 10^7
+    assert b["B3_sort_hist"] + b["B3_sort_pass"] == (8 + 20 + 4 * 24) * n
     assert b["B4_leaves"] == 32 * n
+    assert b["B5B6_hierarchy_refit"] == 92 * n                        # B5 20 + B6 72
     assert b["T2_scan"] == 12 * n + 4
-    assert b["K1K2_knn"] > n * (4 + 12 + 8 * 16)
+    # traversal: per query 4 (order) + 16 (query) + 4 (count); tree = 48 B per TOUCHED primitive
+    t = bench.algorithmic_bytes(cfg, dict(pairs=159_000_000, touched_spatial=460_000, touched_knn=460_000))
+    assert t["T1_spatial_count"] == 2 * (24 * n + 48 * 460_000) + 4 * 159_000_000
+    assert t["K1K2_knn"] == n * (4 + 12 + 8 * 16) + 48 * 460_000     # = 1.46 GB at C3
+    assert b["_whole_tree"] == 4 * (n * 4 + (n - 1) * 16)
+    # boxes (C4) and 5-D points (C5): SURVEY.md's 88 + 20 and 112 + 20 bytes per primitive
+    assert bench.algorithmic_bytes(dict(n=100, nq=10, dim=3, pkind=1, qkind=1, k=None), dict(pairs=0))["B5B6_hierarchy_refit"] == 108 * 100
+    assert bench.algorithmic_bytes(dict(n=100, nq=10, dim=5, pkind=0, qkind=2, k=8), dict(pairs=0))["B5B6_hierarchy_refit"] == 132 * 100
 
 
 def test_reference_arm_prints_contract_line():
@@ -31,7 +40,8 @@ def test_reference_arm_prints_contract_line():
     assert line["impl"] == "reference" and line["unit"] == "queries/s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["value"] == line["value"]
-    assert line["config"]["workload"] == "C1"
+    assert line["config"] == dict(workload="C1", n=10000, nq=10000, dim=3, k=10, r=0.062)
+    assert line["extrapolated_from_queries"] is None and "measured" in line["full_step_source"]
 
 
 _WORKER = r"""

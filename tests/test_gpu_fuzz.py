@@ -21,7 +21,7 @@ def _np(t):
 
 
 @pytest.mark.parametrize("seed", [11, 12, 13])
-def test_random_cases_against_oracle(orc, monkeypatch, seed):
+def test_random_cases_against_oracle(orc, knobs, seed):
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     from oracle import compare as cmp
@@ -32,11 +32,8 @@ def test_random_cases_against_oracle(orc, monkeypatch, seed):
         D = int(rng.integers(1, 11)); pk = int(rng.integers(0, 3)); qk = int(rng.integers(0, 3))
         n = int(rng.choice([1, 2, 5, 33, 700, 5000, 20000])); nq = int(rng.choice([1, 31, 33, 1000, 5000]))
         mode = str(rng.choice(["", "thread", "packet"])); lm = int(rng.choice([1, 4, 16, 16, 64]))
-        monkeypatch.delenv("ARBX_TRAVERSAL", raising=False)
-        if mode:
-            monkeypatch.setenv("ARBX_TRAVERSAL", mode)
-        monkeypatch.setenv("ARBX_LEAF_MAX", str(lm))
-        monkeypatch.setenv("ARBX_STORE_BUDGET_MB", str(rng.choice([0, 1, 4096])))
+        knobs(traversal=mode or None, leaf_max=lm, store_budget_mb=int(rng.choice([0, 1, 4096])),
+              brute_max=int(rng.choice([-1, 0, 0, 1 << 20])))
         ext = 0.5 * (8.0 / max(n, 8)) ** (1.0 / D)
         style = str(rng.choice(["uniform", "clustered", "dups"]))
         s = int(rng.integers(1 << 30))

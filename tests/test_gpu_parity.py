@@ -112,9 +112,9 @@ def test_all_cells_small(arbx, orc, D, pkind):
 
 
 @pytest.mark.parametrize("leaf_max", [1, 2, 8, 64])
-def test_leaf_sizes(arbx, orc, leaf_max, monkeypatch):
+def test_leaf_sizes(arbx, orc, leaf_max, knobs):
     from oracle import compare as cmp
-    monkeypatch.setenv("ARBX_LEAF_MAX", str(leaf_max))
+    knobs(leaf_max=leaf_max)
     prims = dg.uniform_points(5000, 3, 1)
     qp = dg.uniform_points(3000, 3, 2)
     _spatial_case(arbx, orc, cmp, prims, dg.POINT, dg.sphere_queries(qp, 0.08), dg.SPHERE, f"leaf_max={leaf_max}")
@@ -354,15 +354,14 @@ def test_configs_full_sampled(arbx, orc, name):
 # ---- every traversal / CSR-assembly path gives the same answer ------------------------------------------
 @pytest.mark.parametrize("traversal", ["thread", "packet", None])
 @pytest.mark.parametrize("budget_mb", ["0", "1", None])
-def test_paths_agree_with_oracle(arbx, orc, monkeypatch, traversal, budget_mb):
-    """ARBX_TRAVERSAL forces per-lane or packet traversal (default: per-warp choice);
-    ARBX_STORE_BUDGET_MB=0 forces count -> scan -> fill (two traversals), 1 MB gives 16-slot
+def test_paths_agree_with_oracle(arbx, orc, knobs, traversal, budget_mb):
+    """knob traversal forces per-lane or packet traversal (default: per-warp choice);
+    store_budget_mb=0 forces count -> scan -> fill (two traversals), 1 MB gives 16-slot
     stored rows so that dense queries overflow and take the second traversal."""
     from oracle import compare as cmp
-    if traversal:
-        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    knobs(traversal=traversal)
     if budget_mb is not None:
-        monkeypatch.setenv("ARBX_STORE_BUDGET_MB", budget_mb)
+        knobs(store_budget_mb=int(budget_mb))
     prims = dg.uniform_points(6000, 3, 41)
     qp = dg.uniform_points(4000, 3, 42)
     q = dg.sphere_queries(qp, 0.09)          # ~18 hits per query on average: rows above and below 16
@@ -392,10 +391,9 @@ def test_coherent_and_scattered_warps_in_one_batch(arbx, orc):
 
 # ---- NEXT-1: capped count with early exit ----------------------------------------
 @pytest.mark.parametrize("traversal", ["thread", "packet", None])
-def test_count_upto(arbx, orc, monkeypatch, traversal):
+def test_count_upto(arbx, orc, knobs, traversal):
     from oracle import compare as cmp
-    if traversal:
-        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    knobs(traversal=traversal)
     prims = dg.uniform_points(8000, 3, 61)
     q = dg.sphere_queries(dg.uniform_points(5000, 3, 62), 0.08)
     o = orc.spatial(prims, dg.POINT, q, dg.SPHERE)
@@ -451,11 +449,10 @@ def test_run_to_run_determinism(arbx):
 
 
 @pytest.mark.parametrize("traversal", ["thread", "packet", None])
-def test_spatial_upto(arbx, orc, monkeypatch, traversal):
+def test_spatial_upto(arbx, orc, knobs, traversal):
     """Capped storage query (PAPER.md:L174 early exit from a storing callback)."""
     from oracle import compare as cmp
-    if traversal:
-        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    knobs(traversal=traversal)
     prims = dg.uniform_points(8000, 3, 81)
     q = dg.sphere_queries(dg.uniform_points(5000, 3, 82), 0.08)
     o = orc.spatial(prims, dg.POINT, q, dg.SPHERE)
@@ -481,10 +478,9 @@ def test_spatial_upto(arbx, orc, monkeypatch, traversal):
 # ---- NEXT-2: self-join / pair search ------------------------------------------------------
 @pytest.mark.parametrize("traversal", ["thread", "packet", None])
 @pytest.mark.parametrize("D", [2, 3, 5])
-def test_query_pairs(arbx, orc, monkeypatch, traversal, D):
+def test_query_pairs(arbx, orc, knobs, traversal, D):
     from oracle import compare as cmp
-    if traversal:
-        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    knobs(traversal=traversal)
     n = 6000
     p = dg.uniform_points(n, D, 90 + D)
     p[100:140] = p[100]                                      # a clump of duplicates: distance 0 pairs
@@ -516,10 +512,9 @@ def test_query_pairs_lattice_and_errors(arbx):
 # ---- NEXT-3: DBSCAN on top of the index ---------------------------------------
 @pytest.mark.parametrize("traversal", ["thread", "packet", None])
 @pytest.mark.parametrize("D,min_pts", [(2, 5), (3, 4), (3, 1), (5, 6)])
-def test_dbscan(arbx, orc, monkeypatch, traversal, D, min_pts):
+def test_dbscan(arbx, orc, knobs, traversal, D, min_pts):
     from oracle import compare as cmp
-    if traversal:
-        monkeypatch.setenv("ARBX_TRAVERSAL", traversal)
+    knobs(traversal=traversal)
     n = 12000
     blobs = dg.gaussian_mixture(n - 2000, D, 100 + D, centre_seed=7, ncomp=12, sigma=0.015)
     p = np.concatenate([blobs, dg.uniform_points(2000, D, 200 + D)]).astype(np.float32)   # clusters + background noise
