@@ -631,6 +631,8 @@ def main():
         d2h = ho.numel() * 4 + capacity * 4 + hc.numel() * 4 + (hki.numel() * 8 if k else 0)
         assert int(ho[-1]) == capacity and int(hc.sum()) == capacity, "e2e results inconsistent"
     # ---- the other BASELINE.json configurations, same process, after the timed region ------------------
+    l2_note = ("inputs and outputs exceed L2 (no flush needed)" if (d_prims.numel() + d_queries.numel()) * 4 > 126e6
+               else "working set fits L2")
     others = None
     if rank == 0 and world == 1 and not args.no_other_configs and args.scale == 1.0:
         del d_prims, d_queries, d_qpoints, indices, counts, kidx, kdist, offsets
@@ -694,7 +696,7 @@ def main():
                     scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                     config=bench_config(cfg),
                     run=dict(scale=args.scale, parallelism=f"replicas x{world}" if world > 1 else "single GPU",
-                             l2="inputs and outputs exceed L2 (no flush needed)" if (d_prims.numel() + d_queries.numel()) * 4 > 126e6 else "working set fits L2"),
+                             l2=l2_note),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline,
                     cpu_baseline=cpu, breakdown=breakdown, other_configs=others)
         print(json.dumps(line), flush=True)

@@ -340,10 +340,9 @@ class Index:
         entries, padded with -1 / +inf; kmax defaults to max(k))."""
         nq = self._nq(qpoints, POINT)
         per_query = isinstance(k, torch.Tensor)
-        width = int(k) if not per_query else int(kmax if kmax is not None else (int(k.max()) if nq else 1))
-        width = max(width, 1)
-        idx = torch.empty((nq, width), dtype=torch.int32, device=self.device)
-        dist = torch.empty((nq, width), dtype=torch.float32, device=self.device) if want_distances else None
+        width = int(k) if not per_query else max(1, int(kmax if kmax is not None else (int(k.max()) if nq else 1)))
+        idx = torch.empty((nq, max(width, 0)), dtype=torch.int32, device=self.device)
+        dist = torch.empty((nq, max(width, 0)), dtype=torch.float32, device=self.device) if want_distances else None
         if per_query:
             arbx_query_knn_var(self.handle, qpoints, nq, k, width, idx, dist, stream)
         else:

@@ -440,9 +440,12 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
   // capped storage query: capped count (early exit) -> scan -> fill that stops at each count
   if (limit > 0) a.cap = limit;
   a.self = self ? 1 : 0;
+  Scratch<uint32_t> ovf;
   if (cap) {
     ARBX_TRY(rows.alloc((size_t)nq * cap, s));
+    ARBX_TRY(ovf.alloc((size_t)nq, s));
     a.rows = rows.p;
+    a.ovf_list = ovf.p;
   }
   ARBX_TRY(tab->spatial(ix, a, s));
   ARBX_TRY(exclusive_scan_i32(counts.p, offsets, nq, total_dev.p, s));
@@ -472,6 +475,10 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
   if (cap) {
     ARBX_TRY(compact_rows(rows.p, cap, counts.p, offsets, indices, nq, s));
     if (noverflow == 0) return ARBX_OK;
+    // second traversal for the overflowing queries only, packed into dense warps (their order in
+    // the list follows block execution order, so neighbours stay roughly neighbours)
+    // (not for the self-join, whose traversal needs the thread index = the query's leaf position)
+    if (!self) { a.qorder = ovf.p; a.nq = noverflow; }
   }
   return tab->spatial(ix, a, s);
 }

@@ -145,12 +145,13 @@ arbx_status validate_index(const Index* ix, int64_t* violations_host, cudaStream
 // One spatial traversal pass.  pass 0: counts[q] = matches (cap > 0: min(matches, cap), with
 // early exit).  pass 2: the same, and the first
 // `cap` matches of query q are stored in rows[q*cap ..]; *overflow counts the queries with
-// more than cap matches.  pass 1: fill indices[offsets[q] ..]; with cap > 0 only the queries
+// more than cap matches and ovf_list names them (so that pass 1 runs on dense warps).  pass 1: fill indices[offsets[q] ..]; with cap > 0 only the queries
 // whose counts[q] > cap are traversed (the others are copied from rows by compact_rows).
 struct SpatialArgs {
   const float* queries; int64_t nq; int qkind; const uint32_t* qorder;
   int32_t* counts; const int32_t* offsets; int32_t* indices;
   int32_t* rows; int cap; int* overflow; int pass;
+  uint32_t* ovf_list = nullptr;   // pass 2: caller's indices of the queries with more than cap matches
   int stop_fill = 0;   // pass 1 only: query q stops after counts[q] hits (capped storage query)
   int self = 0;        // self-join: query t is the leaf at sorted position t; report later positions only
 };

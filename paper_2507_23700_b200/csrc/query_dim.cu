@@ -351,8 +351,8 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
                                                      int32_t* __restrict__ counts,
                                                      const int32_t* __restrict__ offsets,
                                                      int32_t* __restrict__ indices, int cap,
-                                                     int* __restrict__ overflow, int stop_fill, int mode,
-                                                     float alpha) {
+                                                     int* __restrict__ overflow, uint32_t* __restrict__ ovf_list,
+                                                     int stop_fill, int mode, float alpha) {
   constexpr bool FILL = MODE == 1 || MODE == 2;     // hits are written to rows / CSR slices
   constexpr int QW = prim_width(QK, D);
   constexpr int PQ_CAP = 320;   // packet work list (node ids) per warp
@@ -397,7 +397,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
                                                        capped ? limit : INT32_MAX, (int)t, counts, cap, (int32_t)qi);
     if constexpr (MODE == 0 || MODE == 2) {
       if (valid) counts[qi] = c;
-      if constexpr (MODE == 2) { if (c > cap) atomicAdd(overflow, 1); }
+      if constexpr (MODE == 2) { if (c > cap) ovf_list[atomicAdd(overflow, 1)] = (uint32_t)qi; }
     }
     return;
   }
@@ -518,7 +518,7 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   if constexpr (FILL) flush(__ballot_sync(~0u, pend > 0));
   if constexpr (MODE == 0 || MODE == 2) {
     if (valid) counts[qi] = MODE == 0 ? min(cnt, limit) : cnt;
-    if constexpr (MODE == 2) { if (cnt > cap) atomicAdd(overflow, 1); }
+    if constexpr (MODE == 2) { if (cnt > cap) ovf_list[atomicAdd(overflow, 1)] = (uint32_t)qi; }   // valid: cnt > 0
   }
 }
 
@@ -1059,14 +1059,14 @@ arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s
   if (const float v = g_cfg.packet_alpha.load(std::memory_order_relaxed); v >= 0.f) alpha = v;
   const int n = (int)ix->n;
   if (a.pass == 1)
-    spatial_kernel<PK, QK, 1, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, a.stop_fill, mode, alpha);
+    spatial_kernel<PK, QK, 1, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, nullptr, a.stop_fill, mode, alpha);
   else if (a.pass == 3) {
     if constexpr (SELF)   // DBSCAN edges: counts = neighbour counts (read), rows = union-find array, cap = min_pts
-      spatial_kernel<PK, QK, 3, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, nullptr, 0, mode, alpha);
+      spatial_kernel<PK, QK, 3, true><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, nullptr, nullptr, 0, mode, alpha);
   } else if (a.pass == 2)
-    spatial_kernel<PK, QK, 2, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, 0, mode, alpha);
+    spatial_kernel<PK, QK, 2, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, a.rows, a.cap, a.overflow, a.ovf_list, 0, mode, alpha);
   else
-    spatial_kernel<PK, QK, 0, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, a.cap, nullptr, 0, mode, alpha);
+    spatial_kernel<PK, QK, 0, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, nullptr, nullptr, a.cap, nullptr, nullptr, 0, mode, alpha);
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
@@ -1113,8 +1113,11 @@ arbx_status knn_launch(const Index* ix, const KnnArgs& a, cudaStream_t s) {
   Scratch<uint8_t> flags;
   ARBX_TRY(flags.alloc((size_t)nwarps, s));
   ARBX_CUDA(cudaMemsetAsync(flags.p, 0, (size_t)nwarps, s));
-  float alpha = D <= 3 ? 1.0f : 0.5f;
+  // measured: above 3-D the warps of the clustered workload (C5) are never coherent and the seed
+  // descent is pure overhead (+0.7 ms per 10^7 queries), so packets are off unless asked for
+  float alpha = D <= 3 ? 1.0f : 0.f;
   if (const float v = g_cfg.packet_alpha.load(std::memory_order_relaxed); v >= 0.f) alpha = v;
+  if (alpha <= 0.f && mode != 2) return knn_thread_launch<PK, RegHeap<KB>>(ix, a, nullptr, s);
   const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);
   knn_packet_kernel<PK, KB><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
                                                 reinterpret_cast<const float4*>(ix->leaves), ix->root, (int)ix->n,
