@@ -60,10 +60,14 @@ def _peaks():
 def sort_passes(n, D):
     """8-bit digit passes of the build sort: code width adapted to n (csrc/build.cu, reading A15)."""
     lg = max(0, int(n - 1).bit_length())
-    b = (lg + D - 1) // D + 4
-    passes = (D * b + 7) // 8
-    b = min(min(32, 64 // D), max(b, 8 * passes // D))
+    bmax = min(32, 64 // D)
+    b = min(bmax, (lg + D - 1) // D + 4)
+    b = min(bmax, max(b, 8 * ((D * b + 7) // 8) // D))
     return (D * b + 7) // 8
+
+
+def query_sort_passes(D):
+    return (D * min(16, 32 // D) + 7) // 8
 
 
 def algorithmic_bytes(cfg, totals):
@@ -81,7 +85,7 @@ def algorithmic_bytes(cfg, totals):
                                                                 # (geometry + index, 8-byte granules: 16 / 32 / 24 B for
                                                                 # 3-D points / 3-D boxes / 5-D points; ours pads to 16 B)
     npass = sort_passes(n, D)                                   # 8-bit digit passes, build sort
-    qpass = (D * min(16, 32 // D) + 7) // 8                     # 8-bit digit passes, query sort
+    qpass = query_sort_passes(D)                                # digit passes, query sort
     nbatches = 3 if cfg["k"] else 2                             # query batches per step
     pairs = totals["pairs"]
     per_touched = 4 * lw + 8 * D + 8                            # leaf + child box + links

@@ -399,9 +399,8 @@ arbx_status build_typed(const float* prims, int64_t n, cudaStream_t s, Index* ix
   if (b <= 0) {
     int lg = 0;
     while ((int64_t(1) << lg) < n) ++lg;
-    b = (lg + D - 1) / D + 4;
-    const int passes = (D * b + 7) / 8;
-    b = std::max(b, 8 * passes / D);
+    b = std::min(BMAX, (lg + D - 1) / D + 4);
+    b = std::max(b, 8 * ((D * b + 7) / 8) / D);
   }
   b = std::max(1, std::min(BMAX, b));
   ix->code_bits = b;

@@ -204,13 +204,24 @@ __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes,
                                                int32_t* __restrict__ out, int limit, int stop, int tpos,
                                                const int32_t* __restrict__ counts, int min_pts, int32_t qi) {
   constexpr bool FILL = MODE == 1 || MODE == 2;
+  // Node work and leaf work are separated: a lane that reaches a leaf range does not stop and
+  // wait for the other lanes (measured on C5: the node loop then runs at 5 of 32 lanes), it
+  // queues the range and keeps walking nodes until its stack is empty or its queue is full;
+  // then all lanes scan their queued ranges together.
+  constexpr int LQ = 32;
   int cnt = 0;
   int32_t stack[STACK_DEPTH];
-  int sp = 0;
+  int32_t lq[LQ];
+  int sp = 0, nl = 0;
   constexpr int32_t DONE = INT32_MIN;
   int32_t ref = __ldg(root);
-  for (;;) {   // while-while: descend to a leaf range in every lane, then scan together
-    while (ref >= 0) {
+  for (;;) {
+    while (ref != DONE && nl < LQ) {
+      if (ref < 0) {
+        lq[nl++] = ref;
+        ref = sp > 0 ? stack[--sp] : DONE;
+        continue;
+      }
       NodeX nd;
       load_node_x(nodes, ref, nd);
       bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
@@ -225,20 +236,22 @@ __device__ __forceinline__ int thread_traverse(const float4* __restrict__ nodes,
         ref = sp > 0 ? stack[--sp] : DONE;
       }
     }
-    if (ref == DONE) break;
-    int j = ~ref;
-    for (;; ++j) {
-      Leaf<PK> lf;
-      load_leaf<PK>(leaves, j, lf);
-      if ((!SELF || j > tpos) && hits_prim<QK, PK>(q, lf.v)) {
-        if constexpr (FILL) { if (cnt < limit) out[cnt] = (int32_t)(lf.idx & ~LEAF_END); }
-        if constexpr (MODE == 3) dbscan_edge(out, counts, min_pts, qi, (int32_t)(lf.idx & ~LEAF_END));
-        ++cnt;
-        if (cnt >= stop) return cnt;   // capped query: early exit
+    for (int e = 0; e < nl; ++e) {
+      int j = ~lq[e];
+      for (;; ++j) {
+        Leaf<PK> lf;
+        load_leaf<PK>(leaves, j, lf);
+        if ((!SELF || j > tpos) && hits_prim<QK, PK>(q, lf.v)) {
+          if constexpr (FILL) { if (cnt < limit) out[cnt] = (int32_t)(lf.idx & ~LEAF_END); }
+          if constexpr (MODE == 3) dbscan_edge(out, counts, min_pts, qi, (int32_t)(lf.idx & ~LEAF_END));
+          ++cnt;
+          if (cnt >= stop) return cnt;   // capped query: early exit
+        }
+        if (lf.idx & LEAF_END) break;
       }
-      if (lf.idx & LEAF_END) break;
     }
-    ref = sp > 0 ? stack[--sp] : DONE;
+    nl = 0;
+    if (ref == DONE) break;
   }
   return cnt;
 }
@@ -472,8 +485,26 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
       leaf_range(0, n);
     } else {
       const uint32_t lt = (1u << lane) - 1u;
+      // Upper tree: while only ONE child of the current node can hold a match, and it is an
+      // internal node, there is nothing to spread over the lanes: the warp steps down that
+      // single path (every lane does the same two box tests on a broadcast node) and the work
+      // list starts below it.
+      int32_t top = rootref;
+      for (;;) {
+        NodeX nd;
+        load_node_x(nodes, top, nd);
+        bool h0 = joint_hits_box<QK>(J, nd.v, nd.v + D);
+        bool h1 = joint_hits_box<QK>(J, nd.v + 2 * D, nd.v + 3 * D);
+        if constexpr (SELF) {
+          const int tmin = (int)(t - lane);
+          h0 = h0 && top > tmin; h1 = h1 && nd.r > tmin;
+        }
+        if (h0 && !h1 && nd.c0 >= 0) top = nd.c0;
+        else if (h1 && !h0 && nd.c1 >= 0) top = nd.c1;
+        else break;
+      }
       int nlist = 1;
-      stack[0] = rootref;
+      stack[0] = top;
       __syncwarp();
       while (nlist > 0) {
         const int take = nlist > PQ_CAP - STACK_DEPTH - 64 ? 1 : min(32, nlist);
