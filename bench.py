@@ -526,7 +526,8 @@ def main():
     # hiccup (the storage query synchronises once per call) shows up as max >> median
     begins = [e for (nm, e) in marks if nm == "begin"]
     per_step = [a.elapsed_time(b) for a, b in zip(begins[:-1], begins[1:])] + [begins[-1].elapsed_time(e1)]
-    step_stats = dict(min=round(min(per_step), 4), median=round(float(np.median(per_step)), 4), max=round(max(per_step), 4))
+    step_stats = dict(min=round(min(per_step), 4), median=round(float(np.median(per_step)), 4), max=round(max(per_step), 4),
+                      all=[round(x, 3) for x in per_step])
     marks.clear()
 
     # ---- outside the step: the capped count (NEXT-1, arbx_query_count_upto), device-timed ---------------
