@@ -1146,7 +1146,7 @@ arbx_status knn_launch(const Index* ix, const KnnArgs& a, cudaStream_t s) {
   ARBX_CUDA(cudaMemsetAsync(flags.p, 0, (size_t)nwarps, s));
   // measured: above 3-D the warps of the clustered workload (C5) are never coherent and the seed
   // descent is pure overhead (+0.7 ms per 10^7 queries), so packets are off unless asked for
-  float alpha = D <= 3 ? 1.0f : 0.f;
+  float alpha = D <= 3 ? 2.0f : 0.f;
   if (const float v = g_cfg.packet_alpha.load(std::memory_order_relaxed); v >= 0.f) alpha = v;
   if (alpha <= 0.f && mode != 2) return knn_thread_launch<PK, RegHeap<KB>>(ix, a, nullptr, s);
   const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);

@@ -535,3 +535,50 @@ def test_compare_knn_sphere_tolerance_is_per_pair(orc):
     bad2 = gd.copy(); bad2[0, 1] = np.float32(bad2[0, 1] * (1 + 4e-6))      # 4e-6 relative is far outside eps + slack
     with pytest.raises(AssertionError):
         cmp.compare_knn(s, dg.SPHERE, y, 3, o, (o[0], bad2))
+
+
+# ---- NEXT-4: one k per query -----------------------------------------------------------
+def test_knn_var_lattice_closed_form(orc):
+    """Integer lattice, queries on interior lattice points: k_q = 0 -> an empty (padded) row;
+    k_q = 1 -> the point itself at distance 0; k_q = 2D+1 -> itself + its 2D axis neighbours at
+    distance exactly 1; k_q > kmax is clamped to kmax.  (Worked by hand: the 2D neighbours
+    p +- e_a are the only lattice points at distance 1, the next shell is at sqrt(2).)"""
+    from paper_2507_23700_b200 import datagen as dg
+    for D, g in ((1, 30), (2, 9), (3, 7)):
+        p = dg.lattice_points(g, D)
+        interior = np.nonzero(np.all((p > 0) & (p < g - 1), axis=1))[0]
+        qp = p[interior]
+        kmax = 2 * D + 1
+        kq = np.array([[0, 1, kmax, kmax + 5][i % 4] for i in range(len(interior))], dtype=np.int32)
+        idx, dist = orc.knn_var(p, orc.POINT, qp, kq, kmax)
+        for r, (qi, kk) in enumerate(zip(interior, kq)):
+            kk = min(int(kk), kmax)
+            assert np.all(idx[r, kk:] == -1) and np.all(np.isposinf(dist[r, kk:]))
+            if kk >= 1:
+                assert idx[r, 0] == qi and dist[r, 0] == 0.0
+            if kk == kmax:
+                assert np.all(dist[r, 1:] == 1.0)
+                assert np.all(np.abs(p[idx[r, 1:]] - qp[r]).sum(axis=1) == 1)
+
+
+def test_compare_knn_var_rejects_corruption(orc):
+    from oracle import compare as cmp
+    from paper_2507_23700_b200 import datagen as dg
+    p = dg.uniform_points(400, 3, 5)
+    qp = dg.uniform_points(50, 3, 6)
+    kmax = 6
+    kq = (np.arange(50) % (kmax + 1)).astype(np.int32)
+    o = orc.knn_var(p, orc.POINT, qp, kq, kmax)
+    good = (o[0].copy(), o[1].astype(np.float32))
+    cmp.compare_knn_var(p, orc.POINT, qp, kq, kmax, o, good, what="ok")
+    bad_pad = (good[0].copy(), good[1].copy())
+    r = int(np.nonzero(kq == 2)[0][0])
+    bad_pad[0][r, 3] = 7                                     # an entry past k_q
+    with pytest.raises(AssertionError):
+        cmp.compare_knn_var(p, orc.POINT, qp, kq, kmax, o, bad_pad, what="pad")
+    bad_row = (good[0].copy(), good[1].copy())
+    r = int(np.nonzero(kq == 4)[0][0])
+    far = int(np.argmax(np.linalg.norm(p - qp[r], axis=1)))
+    bad_row[0][r, 3] = far                                   # a wrong neighbour inside the first k_q
+    with pytest.raises(AssertionError):
+        cmp.compare_knn_var(p, orc.POINT, qp, kq, kmax, o, bad_row, what="row")
