@@ -191,7 +191,9 @@ hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict
   constexpr int LW = leaf_width(PK, D);
   constexpr int NW = node_width(D);
   // s_lvl[t] = level of split c0-1+t, t = 0..HB;  s_pre[t] = max s_lvl[0..t];  s_suf[t] = max s_lvl[t..HB]
-  __shared__ uint8_t s_lvl[HB + 1], s_pre[HB + 1], s_suf[HB + 1];
+  constexpr int HALO = 64;   // >= the largest leaf_max
+  __shared__ uint8_t s_lx[HALO + HB + 1 + HALO], s_pre[HB + 1], s_suf[HB + 1];
+  uint8_t* const s_lvl = s_lx + HALO;   // s_lvl[t], -HALO <= t <= HB + HALO
   __shared__ int s_w[HB / 32];
   __shared__ int s_flag[HB];
   __shared__ float s_box[2][HB][2 * D];
@@ -204,11 +206,15 @@ hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict
     s_flag[tid] = -1;
     const int pm = block_running_max<HB>(lv, s_w);
     s_pre[tid] = (uint8_t)pm;
+    if (tid == 0) s_lvl[HB] = (uint8_t)split_level(codes, c0 - 1 + HB, n);
+    __syncthreads();
     // suffix maxima: thread t handles element HB - t (elements HB..1)
-    const int lr = split_level(codes, c0 - 1 + HB - tid, n);
-    if (tid == 0) s_lvl[HB] = (uint8_t)lr;
+    const int lr = s_lvl[HB - tid];
     const int sm = block_running_max<HB>(lr, s_w);
     s_suf[HB - tid] = (uint8_t)sm;
+    // levels of the leaf_max splits on either side of the chunk, for the range classification
+    if (tid < HALO) { if (tid < leaf_max) s_lvl[-1 - tid] = (uint8_t)split_level(codes, c0 - 2 - tid, n); }
+    else if (tid < 2 * HALO) { const int d = tid - HALO; if (d < leaf_max) s_lvl[HB + 1 + d] = (uint8_t)split_level(codes, c0 + HB + d, n); }
   }
   __syncthreads();
 
@@ -230,12 +236,56 @@ hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict
     while (da + db <= leaf_max && lvl(j + db) < L) ++db;
     return da + db > leaf_max;   // subtree size = da + db
   };
+  // the same test for a split of this chunk (0 <= t <= HB), from shared memory only and with a
+  // warp-uniform trip count: nearest level >= L within leaf_max steps on each side
+  auto is_boundary_local = [&](int t) -> bool {
+    const int L = s_lvl[t];
+    if (L == 255) return true;
+    int da = leaf_max + 1, db = leaf_max + 1;
+    for (int d = leaf_max; d >= 1; --d) {
+      if (s_lvl[t - d] >= L) da = d;
+      if (s_lvl[t + d] >= L) db = d;
+    }
+    return da + db > leaf_max;
+  };
   __shared__ uint8_t s_bnd[HB + 1];
-  s_bnd[tid] = is_boundary(c0 - 1 + tid) ? 1 : 0;
-  if (tid == 0) s_bnd[HB] = is_boundary(c0 - 1 + HB) ? 1 : 0;
+  s_bnd[tid] = is_boundary_local(tid) ? 1 : 0;
+  if (tid == 0) s_bnd[HB] = is_boundary_local(HB) ? 1 : 0;
   __syncthreads();
-  if (i >= n || !s_bnd[tid]) return;     // not the first leaf of a range
-  int l = i, r = i;
+  // Every thread loads the box of its own leaf (one coalesced load per thread, all in flight at
+  // once) so that the few range leaders below read shared memory instead of walking global
+  // memory one leaf at a time.
+  constexpr bool STAGE_LEAF = sizeof(float) * 2 * D * HB <= 12288;
+  __shared__ float s_leaf[STAGE_LEAF ? HB : 1][2 * D];
+  if constexpr (STAGE_LEAF) {
+    if (i < n) {
+      float v[W], bl[D], bh[D];
+      const float* lf = leaves + (int64_t)i * LW;
+#pragma unroll
+      for (int e = 0; e < W; ++e) v[e] = lf[e];
+      box_of<D, PK>(v, bl, bh);
+#pragma unroll
+      for (int a = 0; a < D; ++a) { s_leaf[tid][a] = bl[a]; s_leaf[tid][D + a] = bh[a]; }
+    }
+  }
+  // The first leaves of the ranges (about one thread in twelve) are packed into the block's
+  // first warps: the box scans and the climb below then run on full warps instead of on ~3
+  // lanes of every warp.
+  __shared__ uint16_t s_lead[HB];
+  {
+    const bool lead = i < n && s_bnd[tid];
+    const uint32_t bal = __ballot_sync(~0u, lead);
+    const int lane = tid & 31, w = tid >> 5;
+    if (lane == 0) s_w[w] = __popc(bal);
+    __syncthreads();
+    int base = 0, total = 0;
+    for (int k = 0; k < HB / 32; ++k) { const int c = s_w[k]; base += k < w ? c : 0; total += c; }
+    if (lead) s_lead[base + __popc(bal & ((1u << lane) - 1u))] = (uint16_t)tid;
+    __syncthreads();
+    if (tid >= total) return;
+  }
+  const int i0 = c0 + s_lead[tid];
+  int l = i0, r = i0;
   for (;; ++r) {                         // the range ends at the next boundary split
     const int t = r - c0 + 1;
     if (t <= HB ? s_bnd[t] != 0 : is_boundary(r)) break;
@@ -245,11 +295,17 @@ hierarchy_kernel(const unsigned long long* __restrict__ codes, float* __restrict
 #pragma unroll
   for (int a = 0; a < D; ++a) { lo[a] = INFINITY; hi[a] = -INFINITY; }
   for (int j = l; j <= r; ++j) {
-    float v[W], bl[D], bh[D];
-    const float* lf = leaves + (int64_t)j * LW;
+    float bl[D], bh[D];
+    if (STAGE_LEAF && j < c0 + HB) {
 #pragma unroll
-    for (int e = 0; e < W; ++e) v[e] = lf[e];
-    box_of<D, PK>(v, bl, bh);
+      for (int a = 0; a < D; ++a) { bl[a] = s_leaf[j - c0][a]; bh[a] = s_leaf[j - c0][D + a]; }
+    } else {
+      float v[W];
+      const float* lf = leaves + (int64_t)j * LW;
+#pragma unroll
+      for (int e = 0; e < W; ++e) v[e] = lf[e];
+      box_of<D, PK>(v, bl, bh);
+    }
 #pragma unroll
     for (int a = 0; a < D; ++a) { lo[a] = fminf(lo[a], bl[a]); hi[a] = fmaxf(hi[a], bh[a]); }
   }
