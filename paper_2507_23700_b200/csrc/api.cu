@@ -543,7 +543,7 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
     // second traversal for the overflowing queries only, packed into dense warps (their order in
     // the list follows block execution order, so neighbours stay roughly neighbours)
     // (not for the self-join, whose traversal needs the thread index = the query's leaf position)
-    if (!self) { a.qorder = ovf.p; a.nq = noverflow; }
+    if (!self) { a.qorder = ovf.p; a.nq = noverflow; a.heavy = 1; }
   }
   return tab->spatial(ix, a, s);
 }

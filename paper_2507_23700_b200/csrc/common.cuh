@@ -152,6 +152,7 @@ struct SpatialArgs {
   int32_t* counts; const int32_t* offsets; int32_t* indices;
   int32_t* rows; int cap; int* overflow; int pass;
   uint32_t* ovf_list = nullptr;   // pass 2: caller's indices of the queries with more than cap matches
+  int heavy = 0;       // pass 1 only: qorder lists the overflowing queries; one warp per query
   int stop_fill = 0;   // pass 1 only: query q stops after counts[q] hits (capped storage query)
   int self = 0;        // self-join: query t is the leaf at sorted position t; report later positions only
 };

@@ -553,6 +553,89 @@ __global__ void __launch_bounds__(QT) spatial_kernel(const float4* __restrict__ 
   }
 }
 
+// Fill pass for the queries whose row overflowed the stored `cap` hits (list `qlist`, built by
+// MODE 2): ONE WARP PER QUERY.  These are the long rows (hundreds of hits), and a lane walking
+// such a row alone is pure latency (measured: C5 1.3 ms, C4 0.35 ms for a few thousand queries).
+// Here lane i tests the child boxes of node i of a shared-memory work list against the query
+// itself, the primitives of a hit leaf range are tested one per lane, and the hits of a step
+// leave as one ballot-compacted run into the query's CSR slice.
+template <int PK, int QK>
+__global__ void __launch_bounds__(QT) spatial_heavy_kernel(const float4* __restrict__ nodes,
+                                                           const float4* __restrict__ leaves,
+                                                           const int32_t* __restrict__ root, int n,
+                                                           const float* __restrict__ queries,
+                                                           const uint32_t* __restrict__ qlist, int64_t nlistq,
+                                                           const int32_t* __restrict__ offsets,
+                                                           int32_t* __restrict__ indices) {
+  constexpr int QW = prim_width(QK, D);
+  constexpr int PQ_CAP = 320;
+  __shared__ int32_t s_stack[QT / 32][PQ_CAP];
+  int32_t* stack = s_stack[threadIdx.x >> 5];
+  const int lane = threadIdx.x & 31;
+  const int64_t wq = ((int64_t)blockIdx.x * QT + threadIdx.x) >> 5;
+  if (wq >= nlistq) return;
+  const int64_t qi = qlist[wq];
+  Query<QK> q;
+#pragma unroll
+  for (int e = 0; e < QW; ++e) q.v[e] = __ldg(queries + qi * QW + e);
+  if constexpr (QK == KIND_SPHERE) q.r2 = q.v[D] * q.v[D];
+  int64_t base = offsets[qi];
+  const uint32_t lt = (1u << lane) - 1u;
+  auto leaf_range = [&](int first, int m) {   // m is warp-uniform
+    for (int j0 = 0; j0 < m; j0 += 32) {
+      bool hit = false;
+      uint32_t idx = 0;
+      if (j0 + lane < m) {
+        Leaf<PK> lf;
+        load_leaf<PK>(leaves, first + j0 + lane, lf);
+        hit = hits_prim<QK, PK>(q, lf.v);
+        idx = lf.idx & ~LEAF_END;
+      }
+      const uint32_t bal = __ballot_sync(~0u, hit);
+      if (hit) indices[base + __popc(bal & lt)] = (int32_t)idx;
+      base += __popc(bal);
+    }
+  };
+  const int32_t rootref = __ldg(root);
+  if (rootref < 0) { leaf_range(0, n); return; }
+  int nlist = 1;
+  stack[0] = rootref;
+  __syncwarp();
+  while (nlist > 0) {
+    const int take = nlist > PQ_CAP - STACK_DEPTH - 64 ? 1 : min(32, nlist);
+    nlist -= take;
+    const int32_t my = lane < take ? stack[nlist + lane] : -1;
+    __syncwarp();
+    NodeX nd;
+    bool in0 = false, in1 = false, lf0 = false, lf1 = false;
+    if (my >= 0) {
+      load_node_x(nodes, my, nd);
+      const bool h0 = hits_box<QK>(q, nd.v, nd.v + D);
+      const bool h1 = hits_box<QK>(q, nd.v + 2 * D, nd.v + 3 * D);
+      in0 = h0 && nd.c0 >= 0; lf0 = h0 && nd.c0 < 0;
+      in1 = h1 && nd.c1 >= 0; lf1 = h1 && nd.c1 < 0;
+    }
+    uint32_t m0 = __ballot_sync(~0u, lf0), m1 = __ballot_sync(~0u, lf1);
+    while (m0) {
+      const int b = __ffs(m0) - 1;
+      m0 &= m0 - 1;
+      const int l = __shfl_sync(~0u, nd.l, b), p = __shfl_sync(~0u, my, b);
+      leaf_range(l, p - l + 1);
+    }
+    while (m1) {
+      const int b = __ffs(m1) - 1;
+      m1 &= m1 - 1;
+      const int r = __shfl_sync(~0u, nd.r, b), p = __shfl_sync(~0u, my, b);
+      leaf_range(p + 1, r - p);
+    }
+    const uint32_t b0 = __ballot_sync(~0u, in0), b1 = __ballot_sync(~0u, in1);
+    if (in0) stack[nlist + __popc(b0 & lt)] = nd.c0;
+    if (in1) stack[nlist + __popc(b0) + __popc(b1 & lt)] = nd.c1;
+    nlist += __popc(b0) + __popc(b1);
+    __syncwarp();
+  }
+}
+
 // ---- K1 / K2: k nearest neighbours ------------------------------------------------------------------
 // Heap key: squared distance for POINT/BOX primitives, distance for SPHERE primitives
 // (max(0,||y-c||-R) is not monotone in the squared centre distance alone).
@@ -1089,7 +1172,10 @@ arbx_status spatial_launch(const Index* ix, const SpatialArgs& a, cudaStream_t s
   float alpha = D <= 3 ? (QK == KIND_BOX ? 2.5f : 1.5f) : 0.75f;
   if (const float v = g_cfg.packet_alpha.load(std::memory_order_relaxed); v >= 0.f) alpha = v;
   const int n = (int)ix->n;
-  if (a.pass == 1)
+  if (a.pass == 1 && a.heavy && !SELF) {   // qorder = the list of overflowing queries, one warp each
+    const unsigned hgrid = (unsigned)((a.nq * 32 + QT - 1) / QT);
+    spatial_heavy_kernel<PK, QK><<<hgrid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.offsets, a.indices);
+  } else if (a.pass == 1)
     spatial_kernel<PK, QK, 1, SELF><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, n, a.queries, a.qorder, a.nq, a.counts, a.offsets, a.indices, a.cap, nullptr, nullptr, a.stop_fill, mode, alpha);
   else if (a.pass == 3) {
     if constexpr (SELF)   // DBSCAN edges: counts = neighbour counts (read), rows = union-find array, cap = min_pts
