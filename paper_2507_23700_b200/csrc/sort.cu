@@ -22,6 +22,9 @@ constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;   // 4096 elements per tile
 constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_INCL = 2u << 30, VAL_MASK = (1u << 30) - 1;
 constexpr int MAX_PASSES = 8;
 constexpr int SORT_LB = 4;                           // predecessor tiles per look-back round trip
+#ifndef SORT_BLOCKS_PER_SM
+#define SORT_BLOCKS_PER_SM 3
+#endif
 
 __device__ __forceinline__ uint2 ld_volatile_u32x2(const uint2* p) {
   uint2 v;
@@ -116,7 +119,7 @@ __global__ void __launch_bounds__(256) hist_scan_kernel(uint32_t* ghist) {
 // decoupled look-back (two digits per 64-bit status word pair, SORT_LB predecessors per round
 // trip), scatter keys AND values through shared memory in one step, and store them as runs.
 template <typename K, int BITS, bool IOTA, bool VALS>
-__global__ void __launch_bounds__(SORT_THREADS, 2)
+__global__ void __launch_bounds__(SORT_THREADS, SORT_BLOCKS_PER_SM)
 onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* __restrict__ vin,
               uint32_t* __restrict__ vout, uint32_t n, int shift, uint32_t dmask,
               const uint32_t* __restrict__ digit_base, uint32_t* __restrict__ counter,
@@ -135,22 +138,25 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   if (tid == 0) s_tile = atomicAdd(counter, 1u);   // ticket: tile t starts only after tiles < t did
   for (int i = tid; i < SORT_WARPS * HW; i += SORT_THREADS) (&whist[0][0])[i] = 0;
+  static_assert(sizeof(K) * SORT_TILE >= sizeof(uint32_t) * SORT_WARPS * RADIX, "the lane-mask tables borrow the tile");
+  for (int i = tid; i < SORT_WARPS * RADIX; i += SORT_THREADS) reinterpret_cast<uint32_t*>(sort_smem)[i] = 0;
   __syncthreads();
   const uint32_t tile = s_tile;
   const uint32_t tile_base = tile * (uint32_t)SORT_TILE;
   const uint32_t nvalid = min((uint32_t)SORT_TILE, n - tile_base);
 
   // warp-striped load: warp w owns SORT_IPT*32 consecutive elements.  Padding keys of a partial
-  // last tile carry the largest digit of this pass, so they sort behind every real key.
-  K key[SORT_IPT];
-  uint32_t val[SORT_IPT];
+  // last tile carry the largest digit of this pass, so they sort behind every real key.  Only
+  // the DIGITS stay in registers (one byte each): the keys and values are read again for the
+  // scatter, from L2, which keeps the kernel at 40 registers and three resident blocks per SM.
   const uint32_t wbase = tile_base + w * (32 * SORT_IPT) + lane;
   const K pad_key = (K)dmask << shift;
+  uint32_t dig[SORT_IPT];
 #pragma unroll
   for (int j = 0; j < SORT_IPT; ++j) {
-    uint32_t idx = wbase + j * 32;
-    key[j] = idx < n ? kin[idx] : pad_key;
-    if constexpr (VALS) val[j] = IOTA ? idx : (idx < n ? vin[idx] : 0u);
+    const uint32_t idx = wbase + j * 32;
+    const K k = idx < n ? kin[idx] : pad_key;
+    dig[j] = (uint32_t)(k >> shift) & dmask;
   }
 
   // stable rank of every key among the keys of its warp with the same digit.  The match
@@ -158,23 +164,27 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
   // warp keeps item j ahead of item j+1.
   uint16_t rank[SORT_IPT];
   const uint32_t lt_mask = (1u << lane) - 1u;
-  constexpr int MB = 8;
+  // Lanes with the same digit find each other through a per-warp table of lane masks in shared
+  // memory (it borrows the tile's space, which is idle until the scatter): atomicOr of the own
+  // lane bit, read back, the group's first lane clears the entry and bumps the packed counter.
+  // Three shared-memory operations per key where eight ballots + sixteen logic operations were.
+  uint32_t* const wmask = reinterpret_cast<uint32_t*>(sort_smem) + w * RADIX;
 #pragma unroll
-  for (int j0 = 0; j0 < SORT_IPT; j0 += MB) {
-    uint32_t peers[MB];
-#pragma unroll
-    for (int j = 0; j < MB; ++j)
-      peers[j] = match_digit<BITS>((uint32_t)(key[j0 + j] >> shift) & dmask);
-#pragma unroll
-    for (int j = 0; j < MB; ++j) {
-      const uint32_t d = (uint32_t)(key[j0 + j] >> shift) & dmask;
-      const int leader = __ffs(peers[j]) - 1;
-      const int sh16 = (d & 1u) * 16;
-      uint32_t old = 0;
-      if (lane == leader) old = atomicAdd(&whist[w][d >> 1], (uint32_t)__popc(peers[j]) << sh16);
-      old = (__shfl_sync(~0u, old, leader) >> sh16) & 0xffffu;
-      rank[j0 + j] = (uint16_t)(old + __popc(peers[j] & lt_mask));
+  for (int j = 0; j < SORT_IPT; ++j) {
+    const uint32_t d = dig[j];
+    atomicOr(&wmask[d], 1u << lane);
+    __syncwarp();
+    const uint32_t peers = wmask[d];
+    __syncwarp();
+    const int leader = __ffs(peers) - 1;
+    const int sh16 = (d & 1u) * 16;
+    uint32_t old = 0;
+    if (lane == leader) {
+      wmask[d] = 0;
+      old = atomicAdd(&whist[w][d >> 1], (uint32_t)__popc(peers) << sh16);
     }
+    old = (__shfl_sync(~0u, old, leader) >> sh16) & 0xffffu;
+    rank[j] = (uint16_t)(old + __popc(peers & lt_mask));
   }
   __syncthreads();
 
@@ -252,11 +262,12 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
   // scatter keys and values to their position inside the sorted tile, then store runs
 #pragma unroll
   for (int j = 0; j < SORT_IPT; ++j) {
-    const uint32_t d = (uint32_t)(key[j] >> shift) & dmask;
+    const uint32_t idx = wbase + j * 32;
+    const uint32_t d = dig[j];
     const uint32_t wpre = (whist[w][d >> 1] >> ((d & 1u) * 16)) & 0xffffu;
     const uint32_t pos = s_toff[d] + wpre + rank[j];
-    skeys[pos] = key[j];
-    if constexpr (VALS) svals[pos] = val[j];
+    skeys[pos] = idx < n ? __ldcg(kin + idx) : pad_key;
+    if constexpr (VALS) svals[pos] = IOTA ? idx : (idx < n ? __ldcg(vin + idx) : 0u);
   }
   __syncthreads();
 #pragma unroll
