@@ -222,10 +222,15 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
     for (int i = 0; i < SORT_WARPS; ++i) wb += i < w ? s_wsum[i] : 0u;
     x = wb + incl - x;     // first tile position of digit 2*tid
   }
+  const uint32_t toff0 = x, toff1 = x + run0;
   if (tid < HW) {
-    const uint32_t toff0 = x, toff1 = x + run0;
     s_toff[2 * tid] = toff0;
     s_toff[2 * tid + 1] = toff1;
+  }
+  __syncthreads();
+  // The look-back (a few global round trips) is walked by the first HW threads only; the other
+  // warps go straight on to the scatter, which needs s_toff but not the global offsets.
+  if (tid < HW) {
     uint32_t ex0 = 0, ex1 = 0;
     if (tile > 0) {
       // decoupled look-back: SORT_LB predecessors per round trip (independent loads), both digits
@@ -257,7 +262,6 @@ onesweep_pass(const K* __restrict__ kin, K* __restrict__ kout, const uint32_t* _
     s_goff[2 * tid] = digit_base[2 * tid] + ex0 - toff0;
     s_goff[2 * tid + 1] = digit_base[2 * tid + 1] + ex1 - toff1;
   }
-  __syncthreads();
 
   // scatter keys and values to their position inside the sorted tile, then store runs
 #pragma unroll
