@@ -166,6 +166,27 @@ ARBX_API arbx_status arbx_query_knn_var(arbx_handle h, const float* qpoints, int
                                const int32_t* k_per_query, int kmax, int32_t* indices,
                                float* distances, arbx_stream stream);
 
+/* fp64 coordinates (the library "supports different data dimensions (1-10) and
+ * floating point precisions").  Same layouts and semantics as the fp32
+ * calls with `double` rows; kNN distances are fp64.  The results are those of the fp64
+ * predicates / distances evaluated on the caller's fp64 numbers: the index is a tree over the
+ * primitives' bounding boxes rounded OUTWARD to fp32, which only prunes; every reported match or
+ * neighbour is decided by the exact fp64 test at the leaves.  A handle from arbx_build_f64 is
+ * queried with the _f64 calls only (and an fp32 handle with the fp32 calls only): the other
+ * family returns ARBX_ERR_INVALID_ARG.  arbx_size / arbx_destroy / arbx_debug_validate work on
+ * both; arbx_bounds of an fp64 handle gives the fp32 outward-rounded bounds; arbx_query_pairs,
+ * arbx_dbscan, the capped calls and arbx_query_knn_var are fp32 only.  Errors, capacity protocol,
+ * streams and padding as in the fp32 calls.                                                    */
+ARBX_API arbx_status arbx_build_f64(const double* prims, int64_t n, int dim, arbx_kind kind,
+                           arbx_stream stream, arbx_handle* out);
+ARBX_API arbx_status arbx_query_count_f64(arbx_handle h, const double* queries, int64_t nq, arbx_kind qkind,
+                                 int32_t* counts, arbx_stream stream);
+ARBX_API arbx_status arbx_query_spatial_f64(arbx_handle h, const double* queries, int64_t nq, arbx_kind qkind,
+                                   int32_t* offsets, int32_t* indices, int64_t indices_capacity,
+                                   int64_t* total_host, arbx_stream stream);
+ARBX_API arbx_status arbx_query_knn_f64(arbx_handle h, const double* qpoints, int64_t nq, int k,
+                               int32_t* indices, double* distances, arbx_stream stream);
+
 /* Return the library's cached device memory on the current device to the driver, keeping at
  * most keep_bytes (0 = everything not in use).  Does not touch live handles.                 */
 ARBX_API arbx_status arbx_trim(int64_t keep_bytes);

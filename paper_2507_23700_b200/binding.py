@@ -25,6 +25,7 @@ EXPORTS = (
     "arbx_build", "arbx_destroy", "arbx_size", "arbx_bounds", "arbx_query_count",
     "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_spatial_upto", "arbx_query_pairs", "arbx_dbscan", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
     "arbx_query_knn_var", "arbx_trim", "arbx_debug_set",
+    "arbx_build_f64", "arbx_query_count_f64", "arbx_query_spatial_f64", "arbx_query_knn_f64",
     "arbx_launch_count", "arbx_profile_enable", "arbx_profile_num_kernels",
     "arbx_profile_kernel_name", "arbx_profile_read", "arbx_status_string", "arbx_last_error",
 )
@@ -62,6 +63,10 @@ def lib() -> ctypes.CDLL:
         L.arbx_dbscan.argtypes = [vp, ctypes.c_float, i32, vp, vp]
         L.arbx_query_knn.argtypes = [vp, vp, i64, i32, vp, vp, vp]
         L.arbx_query_knn_var.argtypes = [vp, vp, i64, vp, i32, vp, vp, vp]
+        L.arbx_build_f64.argtypes = [vp, i64, i32, i32, vp, ctypes.POINTER(vp)]
+        L.arbx_query_count_f64.argtypes = [vp, vp, i64, i32, vp, vp]
+        L.arbx_query_spatial_f64.argtypes = [vp, vp, i64, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.arbx_query_knn_f64.argtypes = [vp, vp, i64, i32, vp, vp, vp]
         L.arbx_trim.argtypes = [i64]
         L.arbx_debug_set.argtypes = [ctypes.c_char_p, ctypes.c_double]
         L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
@@ -77,7 +82,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_status_string.restype = ctypes.c_char_p
         L.arbx_status_string.argtypes = [i32]
         L.arbx_last_error.restype = ctypes.c_char_p
-        for name in EXPORTS[:16]:
+        for name in EXPORTS[:20]:
             getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -89,11 +94,11 @@ def _stream(stream) -> int:
     return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
 
 
-def _dev_f32(t: torch.Tensor, what: str) -> torch.Tensor:
+def _dev_f32(t: torch.Tensor, what: str, dtype=torch.float32) -> torch.Tensor:
     if not (isinstance(t, torch.Tensor) and t.is_cuda):
         raise TypeError(f"{what} must be a CUDA tensor (no CPU path exists)")
-    if t.dtype != torch.float32 or not t.is_contiguous():
-        raise TypeError(f"{what} must be contiguous float32")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{what} must be contiguous {dtype}")
     return t
 
 
@@ -117,6 +122,36 @@ def arbx_build(prims: torch.Tensor, dim: int, kind: int, stream=None) -> int:
     h = ctypes.c_void_p()
     _check(lib().arbx_build(_ptr(prims), n, dim, kind, _stream(stream), ctypes.byref(h)), "arbx_build")
     return h.value
+
+
+def arbx_build_f64(prims: torch.Tensor, dim: int, kind: int, stream=None) -> int:
+    prims = _dev_f32(prims, "prims", torch.float64)
+    n = prims.numel() // row_width(kind, dim) if prims.numel() else 0
+    h = ctypes.c_void_p()
+    _check(lib().arbx_build_f64(_ptr(prims), n, dim, kind, _stream(stream), ctypes.byref(h)), "arbx_build_f64")
+    return h.value
+
+
+def arbx_query_count_f64(handle: int, queries: torch.Tensor, nq: int, qkind: int, counts: torch.Tensor, stream=None) -> None:
+    _check(lib().arbx_query_count_f64(handle, _ptr(queries), nq, qkind, _ptr(counts), _stream(stream)), "arbx_query_count_f64")
+
+
+def arbx_query_spatial_f64(handle: int, queries: torch.Tensor, nq: int, qkind: int, offsets: torch.Tensor,
+                           indices, capacity: int, stream=None, raise_on_capacity: bool = True):
+    """Returns (status, total)."""
+    total = ctypes.c_int64()
+    st = lib().arbx_query_spatial_f64(handle, _ptr(queries), nq, qkind, offsets.data_ptr(),
+                                      0 if indices is None else indices.data_ptr(), capacity,
+                                      ctypes.byref(total), _stream(stream))
+    if st != OK and (raise_on_capacity or st != ERR_CAPACITY):
+        raise ArbxError(st, "arbx_query_spatial_f64")
+    return st, total.value
+
+
+def arbx_query_knn_f64(handle: int, qpoints: torch.Tensor, nq: int, k: int, indices: torch.Tensor, distances,
+                       stream=None) -> None:
+    _check(lib().arbx_query_knn_f64(handle, _ptr(qpoints), nq, k, _ptr(indices),
+                                    0 if distances is None else _ptr(distances), _stream(stream)), "arbx_query_knn_f64")
 
 
 def arbx_destroy(handle: int, stream=None) -> None:
@@ -245,14 +280,16 @@ class Index:
     """One BVH over `prims` (CUDA float32 [n, row_width]).  PAPER.md:L89-123 (BVH class)."""
 
     def __init__(self, prims: torch.Tensor, kind: int = POINT, dim: int | None = None, stream=None):
-        prims = _dev_f32(prims, "prims")
+        self.f64 = isinstance(prims, torch.Tensor) and prims.dtype == torch.float64
+        self.dtype = torch.float64 if self.f64 else torch.float32
+        prims = _dev_f32(prims, "prims", self.dtype)
         if dim is None:
             if prims.dim() != 2:
                 raise ValueError("give dim= for a flat prims array")
             w = prims.shape[1]
             dim = w if kind == POINT else w // 2 if kind == BOX else w - 1
         self.dim, self.kind, self.device = dim, kind, prims.device
-        self.handle = arbx_build(prims, dim, kind, stream)
+        self.handle = (arbx_build_f64 if self.f64 else arbx_build)(prims, dim, kind, stream)
         self._per_query = 16.0      # matches per query seen so far: sizes the next CSR buffer
 
     def close(self, stream=None):
@@ -276,7 +313,7 @@ class Index:
         return arbx_bounds(self.handle, self.dim, stream)
 
     def _nq(self, queries: torch.Tensor, qkind: int) -> int:
-        _dev_f32(queries, "queries")
+        _dev_f32(queries, "queries", self.dtype)
         return queries.numel() // row_width(qkind, self.dim)
 
     def query_count(self, queries: torch.Tensor, qkind: int = SPHERE, stream=None,
@@ -284,7 +321,11 @@ class Index:
         """counts[q] = matches of query q; with `limit`, min(matches, limit) with early exit."""
         nq = self._nq(queries, qkind)
         counts = torch.empty(nq, dtype=torch.int32, device=self.device)
-        if limit is None:
+        if self.f64:
+            if limit is not None:
+                raise ArbxError(ERR_UNSUPPORTED, "capped count on an fp64 index")
+            arbx_query_count_f64(self.handle, queries, nq, qkind, counts, stream)
+        elif limit is None:
             arbx_query_count(self.handle, queries, nq, qkind, counts, stream)
         else:
             arbx_query_count_upto(self.handle, queries, nq, qkind, limit, counts, stream)
@@ -300,15 +341,15 @@ class Index:
         offsets = torch.empty(nq + 1, dtype=torch.int32, device=self.device)
         if capacity is None:
             capacity = int(nq * self._per_query * 1.25) + 1024
+        call = arbx_query_spatial_f64 if self.f64 else arbx_query_spatial
         indices = torch.empty(capacity, dtype=torch.int32, device=self.device)
-        st, total = arbx_query_spatial(self.handle, queries, nq, qkind, offsets, indices, capacity,
-                                       stream, raise_on_capacity=False)
+        st, total = call(self.handle, queries, nq, qkind, offsets, indices, capacity, stream, raise_on_capacity=False)
         if nq:
             self._per_query = max(1.0, total / nq)
         if st == OK:
             return offsets, indices[:total]
         indices = torch.empty(total, dtype=torch.int32, device=self.device)
-        arbx_query_spatial(self.handle, queries, nq, qkind, offsets, indices, total, stream)
+        call(self.handle, queries, nq, qkind, offsets, indices, total, stream)
         return offsets, indices
 
     def query_spatial_upto(self, queries: torch.Tensor, limit: int, qkind: int = SPHERE, stream=None):
@@ -342,8 +383,12 @@ class Index:
         per_query = isinstance(k, torch.Tensor)
         width = int(k) if not per_query else max(1, int(kmax if kmax is not None else (int(k.max()) if nq else 1)))
         idx = torch.empty((nq, max(width, 0)), dtype=torch.int32, device=self.device)
-        dist = torch.empty((nq, max(width, 0)), dtype=torch.float32, device=self.device) if want_distances else None
-        if per_query:
+        dist = torch.empty((nq, max(width, 0)), dtype=self.dtype, device=self.device) if want_distances else None
+        if self.f64:
+            if per_query:
+                raise ArbxError(ERR_UNSUPPORTED, "per-query k on an fp64 index")
+            arbx_query_knn_f64(self.handle, qpoints, nq, width, idx, dist, stream)
+        elif per_query:
             arbx_query_knn_var(self.handle, qpoints, nq, k, width, idx, dist, stream)
         else:
             arbx_query_knn(self.handle, qpoints, nq, width, idx, dist, stream)

@@ -200,6 +200,7 @@ const DimTable* dim_table(int dim) {
 static void free_index(Index* ix, cudaStream_t s) {
   scratch_free(ix->leaves, s); scratch_free(ix->nodes, s); scratch_free(ix->bounds, s);
   scratch_free(ix->root, s);
+  scratch_free(ix->rows64, s);
 }
 
 // Q1 + Q2: order in which the queries are traversed (neighbours on the curve share a warp)
@@ -381,6 +382,7 @@ static arbx_status count_impl(arbx_handle h, const float* queries, int64_t nq, a
     set_error("arbx_query_count: invalid argument");
     return ARBX_ERR_INVALID_ARG;
   }
+  if (h->ix.f64) { set_error("arbx_query_count: the handle was built from fp64 coordinates, use the _f64 calls"); return ARBX_ERR_INVALID_ARG; }
   if (nq > kMaxCount) { set_error("arbx_query_count: nq > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
   if (nq == 0) return ARBX_OK;
   cudaStream_t s = (cudaStream_t)stream;
@@ -413,7 +415,7 @@ arbx_status arbx_query_spatial_upto(arbx_handle h, const float* queries, int64_t
 arbx_status arbx_query_pairs(arbx_handle h, float radius, int32_t* offsets, int32_t* indices,
                              int64_t indices_capacity, int64_t* total_host, arbx_stream stream) {
   if (!h || !(radius >= 0.f)) { set_error("arbx_query_pairs: invalid argument"); return ARBX_ERR_INVALID_ARG; }
-  if (h->ix.kind != KIND_POINT) { set_error("arbx_query_pairs: POINT primitives only"); return ARBX_ERR_UNSUPPORTED; }
+  if (h->ix.kind != KIND_POINT || h->ix.f64) { set_error("arbx_query_pairs: fp32 POINT primitives only"); return ARBX_ERR_UNSUPPORTED; }
   return spatial_impl(h, nullptr, h->ix.n, ARBX_SPHERE, 0, offsets, indices, indices_capacity, total_host, stream, radius);
 }
 
@@ -423,7 +425,7 @@ arbx_status arbx_dbscan(arbx_handle h, float eps, int32_t min_pts, int32_t* labe
     return ARBX_ERR_INVALID_ARG;
   }
   const Index* ix = &h->ix;
-  if (ix->kind != KIND_POINT) { set_error("arbx_dbscan: POINT primitives only"); return ARBX_ERR_UNSUPPORTED; }
+  if (ix->kind != KIND_POINT || ix->f64) { set_error("arbx_dbscan: fp32 POINT primitives only"); return ARBX_ERR_UNSUPPORTED; }
   const int64_t n = ix->n;
   if (n == 0) return ARBX_OK;
   cudaStream_t s = (cudaStream_t)stream;
@@ -463,6 +465,7 @@ static arbx_status spatial_impl(arbx_handle h, const float* queries, int64_t nq,
     set_error("arbx_query_spatial: invalid argument");
     return ARBX_ERR_INVALID_ARG;
   }
+  if (h->ix.f64) { set_error("arbx_query_spatial: the handle was built from fp64 coordinates, use the _f64 calls"); return ARBX_ERR_INVALID_ARG; }
   if (nq > kMaxCount) { set_error("arbx_query_spatial: nq > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
   cudaStream_t s = (cudaStream_t)stream;
   const Index* ix = &h->ix;
@@ -554,6 +557,7 @@ static arbx_status knn_impl(arbx_handle h, const float* qpoints, int64_t nq, con
     set_error("%s: invalid argument", who);
     return ARBX_ERR_INVALID_ARG;
   }
+  if (h->ix.f64) { set_error("%s: the handle was built from fp64 coordinates, use the _f64 calls", who); return ARBX_ERR_INVALID_ARG; }
   if (k > ARBX_K_MAX) { set_error("%s: k=%d > ARBX_K_MAX=%d", who, k, ARBX_K_MAX); return ARBX_ERR_UNSUPPORTED; }
   if (nq > kMaxCount) { set_error("%s: nq > 2^30 unsupported", who); return ARBX_ERR_UNSUPPORTED; }
   if (nq == 0) return ARBX_OK;
@@ -580,6 +584,119 @@ arbx_status arbx_query_knn_var(arbx_handle h, const float* qpoints, int64_t nq, 
                                int kmax, int32_t* indices, float* distances, arbx_stream stream) {
   if (nq > 0 && !k_per_query) { set_error("arbx_query_knn_var: null k_per_query"); return ARBX_ERR_INVALID_ARG; }
   return knn_impl(h, qpoints, nq, k_per_query, kmax, indices, distances, stream, "arbx_query_knn_var");
+}
+
+// ---- fp64 coordinates (NEXT-4): exact fp64 leaf tests over the fp32 tree, see f64.cu ----------------
+arbx_status arbx_build_f64(const double* prims, int64_t n, int dim, arbx_kind kind, arbx_stream stream,
+                           arbx_handle* out) {
+  if (!out || n < 0 || dim < 1 || dim > ARBX_MAX_DIM || bad_kind((int)kind) || (n > 0 && !prims)) {
+    set_error("arbx_build_f64: invalid argument (n=%lld dim=%d kind=%d)", (long long)n, dim, (int)kind);
+    return ARBX_ERR_INVALID_ARG;
+  }
+  if (n > kMaxCount) { set_error("arbx_build_f64: n > 2^30 unsupported"); return ARBX_ERR_UNSUPPORTED; }
+  cudaStream_t s = (cudaStream_t)stream;
+  arbx_index_s* h = new arbx_index_s();
+  h->ix.leaf_max = std::max(1, std::min(64, g_cfg.leaf_max.load(std::memory_order_relaxed)));
+  arbx_status st = f64_build(prims, n, dim, (int)kind, s, &h->ix);
+  if (st != ARBX_OK) {
+    free_index(&h->ix, s);
+    delete h;
+    return st;
+  }
+  *out = h;
+  return ARBX_OK;
+}
+
+static arbx_status f64_query_prologue(arbx_handle h, const double* queries, int64_t nq, int qkind, const char* who,
+                                      Scratch<float>& qboxes, QueryOrder& order, cudaStream_t s) {
+  if (!h->ix.f64) { set_error("%s: the handle was built from fp32 coordinates", who); return ARBX_ERR_INVALID_ARG; }
+  if (nq > kMaxCount) { set_error("%s: nq > 2^30 unsupported", who); return ARBX_ERR_UNSUPPORTED; }
+  ARBX_TRY(qboxes.alloc((size_t)nq * 2 * h->ix.dim, s));
+  ARBX_TRY(f64_qboxes(queries, nq, h->ix.dim, qkind, qboxes.p, s));
+  return query_order(&h->ix, qboxes.p, nq, KIND_BOX, order, s);   // the curve order of the fp32 boxes
+}
+
+arbx_status arbx_query_count_f64(arbx_handle h, const double* queries, int64_t nq, arbx_kind qkind,
+                                 int32_t* counts, arbx_stream stream) {
+  if (!h || nq < 0 || bad_kind((int)qkind) || (nq > 0 && (!queries || !counts))) {
+    set_error("arbx_query_count_f64: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  if (nq == 0) return ARBX_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (h->ix.f64 && h->ix.n == 0) { ARBX_CUDA(cudaMemsetAsync(counts, 0, (size_t)nq * sizeof(int32_t), s)); return ARBX_OK; }
+  Scratch<float> qboxes;
+  QueryOrder order;
+  ARBX_TRY(f64_query_prologue(h, queries, nq, (int)qkind, "arbx_query_count_f64", qboxes, order, s));
+  return f64_spatial(&h->ix, queries, qboxes.p, order.p, nq, (int)qkind, counts, nullptr, nullptr, 0, s);
+}
+
+arbx_status arbx_query_spatial_f64(arbx_handle h, const double* queries, int64_t nq, arbx_kind qkind,
+                                   int32_t* offsets, int32_t* indices, int64_t indices_capacity,
+                                   int64_t* total_host, arbx_stream stream) {
+  if (!h || nq < 0 || bad_kind((int)qkind) || !offsets || (nq > 0 && !queries) || indices_capacity < 0) {
+    set_error("arbx_query_spatial_f64: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  if (total_host) *total_host = 0;
+  if (nq == 0 || (h->ix.f64 && h->ix.n == 0)) {
+    if (!h->ix.f64) { set_error("arbx_query_spatial_f64: the handle was built from fp32 coordinates"); return ARBX_ERR_INVALID_ARG; }
+    ARBX_CUDA(cudaMemsetAsync(offsets, 0, (size_t)(nq + 1) * sizeof(int32_t), s));
+    return ARBX_OK;
+  }
+  Scratch<float> qboxes;
+  QueryOrder order;
+  ARBX_TRY(f64_query_prologue(h, queries, nq, (int)qkind, "arbx_query_spatial_f64", qboxes, order, s));
+  Scratch<int32_t> counts;
+  Scratch<long long> total_dev;
+  ARBX_TRY(counts.alloc((size_t)nq, s));
+  ARBX_TRY(total_dev.alloc(2, s));
+  ARBX_CUDA(cudaMemsetAsync(total_dev.p, 0, 2 * sizeof(long long), s));
+  ARBX_TRY(f64_spatial(&h->ix, queries, qboxes.p, order.p, nq, (int)qkind, counts.p, nullptr, nullptr, 0, s));
+  ARBX_TRY(exclusive_scan_i32(counts.p, offsets, nq, total_dev.p, s));
+  long long total = 0;
+  int32_t rootw[2] = {0, 0};
+  ARBX_CUDA(cudaMemcpyAsync(&total, total_dev.p, sizeof(total), cudaMemcpyDeviceToHost, s));
+  ARBX_CUDA(cudaMemcpyAsync(rootw, h->ix.root, sizeof(rootw), cudaMemcpyDeviceToHost, s));
+  ARBX_CUDA(cudaStreamSynchronize(s));
+  ARBX_TRY(check_build_fault(rootw[1]));
+  if (total_host) *total_host = total;
+  if (total > 0x7fffffffLL) { set_error("arbx_query_spatial_f64: total %lld exceeds INT32_MAX", total); return ARBX_ERR_OVERFLOW; }
+  if (!indices) return ARBX_OK;
+  if (indices_capacity < total) {
+    set_error("arbx_query_spatial_f64: capacity %lld < total %lld", (long long)indices_capacity, total);
+    return ARBX_ERR_CAPACITY;
+  }
+  if (total == 0) return ARBX_OK;
+  return f64_spatial(&h->ix, queries, qboxes.p, order.p, nq, (int)qkind, nullptr, offsets, indices, 1, s);
+}
+
+__global__ void fill_knn_empty_f64_kernel(int32_t* idx, double* dist, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    idx[i] = -1;
+    if (dist) dist[i] = INFINITY;
+  }
+}
+
+arbx_status arbx_query_knn_f64(arbx_handle h, const double* qpoints, int64_t nq, int k, int32_t* indices,
+                               double* distances, arbx_stream stream) {
+  if (!h || nq < 0 || k < 1 || (nq > 0 && (!qpoints || !indices))) {
+    set_error("arbx_query_knn_f64: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  if (k > ARBX_K_MAX) { set_error("arbx_query_knn_f64: k=%d > ARBX_K_MAX=%d", k, ARBX_K_MAX); return ARBX_ERR_UNSUPPORTED; }
+  if (nq == 0) return ARBX_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (h->ix.f64 && h->ix.n == 0) {
+    fill_knn_empty_f64_kernel<<<256, 256, 0, s>>>(indices, distances, nq * k);
+    ARBX_LAUNCH_CHECK();
+    return ARBX_OK;
+  }
+  Scratch<float> qboxes;
+  QueryOrder order;
+  ARBX_TRY(f64_query_prologue(h, qpoints, nq, KIND_POINT, "arbx_query_knn_f64", qboxes, order, s));
+  return f64_knn(&h->ix, qpoints, order.p, nq, k, indices, distances, s);
 }
 
 arbx_status arbx_sort_pairs(void* keys, uint32_t* values, int64_t n, int key_bytes, int key_bits,

@@ -48,6 +48,11 @@ struct Index {
   float* nodes = nullptr;       // max(n-1,0) * node_width floats
   float* bounds = nullptr;      // 2*dim floats: lo[dim], hi[dim] of all primitives
   int32_t* root = nullptr;      // 2 ints (device): [0] root child ref, [1] build fault flags
+  // fp64 coordinates (f64.cu): the tree is a BOX tree over outward-rounded fp32 boxes; the fp64
+  // rows of the caller's kind `kind64` sit beside it in leaf order
+  bool f64 = false;
+  int kind64 = 0;
+  double* rows64 = nullptr;
 };
 constexpr int BUILD_FAULT_OPEN_OVERFLOW = 1;   // hierarchy: more parked subtrees than open_cap
 
@@ -168,6 +173,14 @@ using qcode_fn = arbx_status (*)(const Index*, const float* queries, int64_t nq,
                                  uint32_t* codes, int* key_bits, cudaStream_t);
 struct DimTable { spatial_fn spatial; knn_fn knn; qcode_fn qcode; };
 const DimTable* dim_table(int dim);
+
+// f64.cu: fp64 coordinates as exact fp64 leaf tests over the fp32 tree
+arbx_status f64_build(const double* prims, int64_t n, int dim, int kind, cudaStream_t s, Index* ix);
+arbx_status f64_qboxes(const double* queries, int64_t nq, int dim, int qkind, float* qboxes, cudaStream_t s);
+arbx_status f64_spatial(const Index* ix, const double* queries, const float* qboxes, const uint32_t* qorder, int64_t nq,
+                        int qkind, int32_t* counts, const int32_t* offsets, int32_t* indices, int fill, cudaStream_t s);
+arbx_status f64_knn(const Index* ix, const double* qpoints, const uint32_t* qorder, int64_t nq, int k, int32_t* indices,
+                    double* distances, cudaStream_t s);
 
 // scan.cu: offsets[0..nq] = exclusive scan of counts[0..nq); *total (device, int64) = sum
 arbx_status exclusive_scan_i32(const int32_t* counts, int32_t* offsets, int64_t nq,

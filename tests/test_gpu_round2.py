@@ -334,3 +334,107 @@ def _full_elementwise(arbx, orc, name, chunk=1_000_000):
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
 def test_configs_full_elementwise(arbx, orc, name):
     _full_elementwise(arbx, orc, name)
+
+
+# ---- NEXT-4: fp64 coordinates ---------------------------------------------------------------
+def _f64_prims(kind, n, D, seed, ext):
+    """fp64 inputs that are NOT representable in fp32: fp32-scale coordinates plus offsets far below
+    the fp32 resolution, on top of a large common shift (1000) where fp32 resolves only ~6e-5."""
+    g = np.random.default_rng(seed)
+    c = 1000.0 + g.random((n, D))
+    if kind == dg.POINT:
+        return c
+    if kind == dg.BOX:
+        w = ext * (0.5 + g.random((n, D)))
+        return np.concatenate([c - w, c + w], axis=1)
+    return np.concatenate([c, ext * (0.5 + g.random((n, 1)))], axis=1)
+
+
+@pytest.mark.parametrize("D", [1, 3, 6])
+@pytest.mark.parametrize("pkind", [dg.POINT, dg.BOX, dg.SPHERE])
+def test_f64_coordinates_against_fp64_oracle(arbx, knobs, D, pkind):
+    """Every (query kind x primitive kind) cell and kNN on fp64 inputs whose structure lies BELOW
+    fp32 resolution (coordinates ~1000 with features of size ~1e-2 .. 1e-6): an fp32 path could
+    not answer these; the fp64 path must match the fp64 oracle (oracle/f64.py)."""
+    from oracle import compare as cmp, f64
+    from test_gpu_parity import _np
+    knobs(brute_max=0)
+    n, nq = 6000, 1200
+    ext = 0.5 * (8.0 / n) ** (1.0 / D)
+    prims = _f64_prims(pkind, n, D, 70 + D, ext)
+    g = np.random.default_rng(90 + D)
+    qp = 1000.0 + g.random((nq, D))
+    qp[: nq // 4] = prims[: nq // 4, :D] + 1e-7 * g.standard_normal((nq // 4, D))     # far below fp32 resolution
+    cases = [(dg.SPHERE, np.concatenate([qp, np.full((nq, 1), ext * 1.3)], axis=1)),
+             (dg.BOX, np.concatenate([qp - ext, qp + ext], axis=1)),
+             (dg.POINT, np.concatenate([qp[: nq // 2], prims[: nq - nq // 2, :D]], axis=0))]
+    ix = arbx.Index(torch.from_numpy(prims).cuda(), pkind, dim=D)
+    assert ix.f64 and ix.validate() == 0 and ix.size() == n
+    for qkind, q in cases:
+        dq = torch.from_numpy(np.ascontiguousarray(q)).cuda()
+        counts = _np(ix.query_count(dq, qkind))
+        off, idx = ix.query_spatial(dq, qkind)
+        o = f64.spatial(prims, pkind, q, qkind)
+        cmp.compare_spatial(n, o, (_np(off), _np(idx)), f"f64 D={D} pk={pkind} qk={qkind}")
+        cmp.compare_counts(o, counts, f"f64 counts D={D} pk={pkind} qk={qkind}")
+        assert np.array_equal(counts, np.diff(_np(off)))
+    for k in (1, 8, 40):
+        gi, gd = ix.query_knn(torch.from_numpy(qp).cuda(), k)
+        gi, gd = _np(gi), _np(gd)
+        oi, od = f64.knn(prims, pkind, qp, k)
+        assert gd.dtype == np.float64 and np.all(np.diff(gd, axis=1) >= 0)
+        assert np.allclose(gd, od, rtol=1e-12, atol=1e-12)            # fp64 agreement, far inside 1e-6
+        dm = f64.knn_distance_matrix(prims, pkind, qp)
+        assert np.allclose(np.take_along_axis(dm, gi.astype(np.int64), axis=1), gd, rtol=1e-12, atol=1e-12)
+        assert np.all(np.sort(gi, axis=1)[:, 1:] != np.sort(gi, axis=1)[:, :-1]) if k > 1 else True
+    ix.close()
+
+
+def test_f64_resolves_what_fp32_cannot(arbx):
+    """Points 1e-6 apart at coordinate 1000 collapse in fp32 (resolution 6e-5); the fp64 index keeps
+    them apart: radius 1.5e-6 around point i of a line of points spaced 1e-6 finds exactly i-1, i, i+1."""
+    n = 2000
+    x = 1000.0 + 1e-6 * np.arange(n)
+    prims = np.stack([x, np.zeros(n), np.zeros(n)], axis=1)
+    ix = arbx.Index(torch.from_numpy(prims).cuda(), dg.POINT)
+    q = np.concatenate([prims, np.full((n, 1), 1.5e-6)], axis=1)
+    off, idx = ix.query_spatial(torch.from_numpy(q).cuda(), dg.SPHERE)
+    off, idx = off.cpu().numpy(), idx.cpu().numpy()
+    assert np.array_equal(np.diff(off)[1:-1], np.full(n - 2, 3)) and np.diff(off)[0] == 2 and np.diff(off)[-1] == 2
+    for i in (1, 500, n - 2):
+        assert sorted(idx[off[i]:off[i + 1]].tolist()) == [i - 1, i, i + 1]
+    gi, gd = ix.query_knn(torch.from_numpy(prims[10:20]).cuda(), 3)
+    assert np.allclose(gd.cpu().numpy()[:, 1:], 1e-6, rtol=1e-6) and np.all(gd.cpu().numpy()[:, 0] == 0)
+    ix.close()
+
+
+def test_f64_edges_and_type_checks(arbx):
+    p64 = torch.from_numpy(1000.0 + np.random.default_rng(1).random((300, 3))).cuda()
+    p32 = p64.float()
+    q64 = torch.cat([p64[:50], torch.full((50, 1), 0.1, dtype=torch.float64, device="cuda")], dim=1).contiguous()
+    ix64, ix32 = arbx.Index(p64, dg.POINT), arbx.Index(p32, dg.POINT)
+    cnt = torch.empty(50, dtype=torch.int32, device="cuda")
+    with pytest.raises(arbx.ArbxError):
+        arbx.arbx_query_count_f64(ix32.handle, q64, 50, dg.SPHERE, cnt)           # fp32 handle, fp64 call
+    with pytest.raises(arbx.ArbxError):
+        arbx.arbx_query_count(ix64.handle, q64.float().contiguous(), 50, dg.SPHERE, cnt)   # fp64 handle, fp32 call
+    with pytest.raises(arbx.ArbxError):
+        arbx.arbx_query_pairs(ix64.handle, 0.1, torch.empty(301, dtype=torch.int32, device="cuda"), None, 0)
+    # brute-force fp64 index (n <= 512 by default) equals the tree-based one
+    c1 = ix64.query_count(q64, dg.SPHERE)
+    arbx.arbx_debug_set("brute_max", 0)
+    ix64t = arbx.Index(p64, dg.POINT)
+    arbx.arbx_debug_set("reset", 0)
+    assert torch.equal(c1, ix64t.query_count(q64, dg.SPHERE)) and int(c1.sum()) > 50
+    # empty index, nq = 0, n < k padding
+    e = arbx.Index(torch.empty((0, 3), dtype=torch.float64, device="cuda"), dg.POINT, dim=3)
+    assert e.empty() and int(e.query_count(q64, dg.SPHERE).sum()) == 0
+    gi, gd = e.query_knn(p64[:5].contiguous(), 4)
+    assert torch.all(gi == -1) and torch.all(torch.isinf(gd))
+    small = arbx.Index(p64[:2].contiguous(), dg.POINT)
+    gi, gd = small.query_knn(p64[:5].contiguous(), 4)
+    assert torch.all(gi[:, 2:] == -1) and torch.all(gi[:, :2] >= 0) and torch.all(torch.isinf(gd[:, 2:]))
+    off0, idx0 = ix64.query_spatial(torch.empty((0, 4), dtype=torch.float64, device="cuda"), dg.SPHERE)
+    assert off0.cpu().tolist() == [0]
+    for ix in (ix64, ix32, ix64t, e, small):
+        ix.close()

@@ -582,3 +582,46 @@ def test_compare_knn_var_rejects_corruption(orc):
     bad_row[0][r, 3] = far                                   # a wrong neighbour inside the first k_q
     with pytest.raises(AssertionError):
         cmp.compare_knn_var(p, orc.POINT, qp, kq, kmax, o, bad_row, what="row")
+
+
+# ---- NEXT-4: fp64 coordinates (oracle/f64.py) ---------------------------------------------------------
+def test_f64_oracle_lattice_closed_forms():
+    """The fp64 oracle against the lattice closed forms (worked by hand): radius 1 around an
+    interior lattice point = itself + its 2D axis neighbours; radius 2 in 3-D = 33 points;
+    k = 2D+1 nearest = the same 2D+1 points at distances 0 and 1."""
+    from oracle import f64
+    from paper_2507_23700_b200 import datagen as dg
+    for D, g in ((1, 20), (2, 9), (3, 7)):
+        p = dg.lattice_points(g, D).astype(np.float64)
+        interior = np.nonzero(np.all((p > 0) & (p < g - 1), axis=1))[0]
+        q = np.concatenate([p[interior], np.ones((len(interior), 1))], axis=1)
+        off, idx, band = f64.spatial(p, f64.POINT, q, f64.SPHERE)
+        assert np.all(np.diff(off) == 2 * D + 1)               # d^2 = 1 <= 1: closed (band or sure)
+        ki, kd = f64.knn(p, f64.POINT, p[interior], 2 * D + 1)
+        assert np.array_equal(ki[:, 0], interior) and np.all(kd[:, 0] == 0) and np.all(kd[:, 1:] == 1.0)
+    p = dg.lattice_points(7, 3).astype(np.float64)
+    c = np.array([[3.0, 3.0, 3.0, 2.0]])
+    assert np.diff(f64.spatial(p, f64.POINT, c, f64.SPHERE)[0])[0] == 33
+
+
+@pytest.mark.parametrize("pk", [0, 1, 2])
+@pytest.mark.parametrize("qk", [0, 1, 2])
+def test_f64_oracle_equals_cpp_oracle_on_fp32_inputs(orc, pk, qk):
+    """On inputs that are exactly representable in fp32 the two oracles do the same fp64
+    arithmetic on the same numbers: rows, bands and kNN index rows must be identical, distances
+    equal up to the order of the fp64 sums."""
+    from oracle import f64
+    from paper_2507_23700_b200 import datagen as dg
+    D, n, nq = 3, 600, 150
+    ext = 0.5 * (8.0 / n) ** (1.0 / D)
+    p = {0: dg.uniform_points(n, D, 3), 1: dg.uniform_boxes(n, D, 3, ext), 2: dg.uniform_spheres(n, D, 3, ext)}[pk]
+    qp = dg.uniform_points(nq, D, 4)
+    q = {2: dg.sphere_queries(qp, ext * 1.4), 1: dg.uniform_boxes(nq, D, 5, ext),
+         0: np.concatenate([qp[: nq // 2], p[: nq - nq // 2, :D]], axis=0)}[qk]
+    a = orc.spatial(p, pk, q, qk)
+    b = f64.spatial(p.astype(np.float64), pk, q.astype(np.float64), qk)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    ka = orc.knn(p, pk, qp, 7)
+    kb = f64.knn(p.astype(np.float64), pk, qp.astype(np.float64), 7)
+    assert np.array_equal(ka[0], kb[0])
+    assert np.allclose(ka[1], kb[1], rtol=1e-13, atol=0.0)      # same numbers up to the order of the fp64 sums
