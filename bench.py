@@ -566,6 +566,23 @@ def main():
             extras["self_join_prims_per_s"] = round(n / a.elapsed_time(b) * 1e3, 1)
             del poff, pidx
         arbx.arbx_destroy(hx, stream)
+        # NEXT-4 fp64 coordinates (arbx_*_f64: exact fp64 leaf tests over the fp32 tree), device-timed on
+        # the same primitives and the first 10^6 queries of the batch, converted to fp64
+        nq64 = min(nq, 1_000_000)
+        p64, q64 = d_prims.double(), d_queries[:nq64].double().contiguous()
+        c64 = torch.empty(nq64, dtype=torch.int32, device=dev)
+        for rep in range(2):
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True); c = torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            h64 = arbx.arbx_build_f64(p64, D, pk, stream)
+            b.record(stream)
+            arbx.arbx_query_count_f64(h64, q64, nq64, qk, c64, stream)
+            c.record(stream)
+            arbx.arbx_destroy(h64, stream)
+        torch.cuda.synchronize()
+        extras["f64_build_mprims_s"] = round(n / a.elapsed_time(b) / 1e3, 2)
+        extras["f64_count_qps"] = round(nq64 / b.elapsed_time(c) * 1e3, 1)
+        del p64, q64, c64
     torch.cuda.synchronize()
 
     # ---- e2e leg: pinned host inputs in, every result back to pinned host memory ---------------------
