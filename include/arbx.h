@@ -199,7 +199,8 @@ ARBX_API arbx_status arbx_trim(int64_t keep_bytes);
  * count -> scan -> fill), "traversal" (0 = per-warp choice, 1 = one query per lane, 2 =
  * warp packets), "packet_alpha" (packet threshold, < 0 = default), "qbits" (query-code bits
  * per axis used by the query sort, 0 = all), "l2_persist" (1 = persisting-L2 window over the
- * node array during queries), "pool_keep_mb" (release threshold of the memory pool),
+ * node array during queries), "gather" (1 = arbx_query_count copies the queries into sorted order
+ * first and un-permutes the counts), "pool_keep_mb" (release threshold of the memory pool),
  * "reset" (all knobs back to their defaults).  Results never depend on these knobs; they
  * choose between equivalent paths.  ARBX_ERR_INVALID_ARG for an unknown key.                 */
 ARBX_API arbx_status arbx_debug_set(const char* key, double value);

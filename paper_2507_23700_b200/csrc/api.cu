@@ -273,6 +273,21 @@ __global__ void fill_knn_empty_kernel(int32_t* idx, float* dist, int64_t n) {
   }
 }
 
+// Q3 experiment (knob "gather"): sorted[t] = queries[order[t]] (rows of w floats), and the inverse
+// for the counts: counts[order[t]] = sorted_counts[t]
+__global__ void gather_rows_kernel(const float* __restrict__ rows, const uint32_t* __restrict__ order, int64_t nq, int w,
+                                   float* __restrict__ sorted) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nq * w) return;
+  const int64_t t = e / w;
+  sorted[e] = rows[(int64_t)order[t] * w + (e - t * w)];
+}
+__global__ void unpermute_i32_kernel(const int32_t* __restrict__ sorted, const uint32_t* __restrict__ order, int64_t nq,
+                                     int32_t* __restrict__ out) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < nq) out[order[t]] = sorted[t];
+}
+
 // self-join queries: query i = (point i, radius) in the caller's order; order[t] = caller's
 // index of the leaf at sorted position t (so no query sort is needed: tree order IS the order)
 __global__ void self_queries_kernel(const float* __restrict__ leaves, int64_t n, int D, int LW, float radius,
@@ -392,6 +407,22 @@ static arbx_status count_impl(arbx_handle h, const float* queries, int64_t nq, a
   ARBX_TRY(query_order(ix, queries, nq, (int)qkind, order, s));
   SpatialArgs a{queries, nq, (int)qkind, order.p, counts, nullptr, nullptr, nullptr, limit, nullptr, 0};
   L2Window l2(ix, s);
+  if (g_cfg.gather.load(std::memory_order_relaxed) && order.p) {
+    // Q3 materialised (experiment): sorted copy of the queries, counts written in
+    // sorted order, then un-permuted
+    const int w = prim_width((int)qkind, ix->dim);
+    Scratch<float> sq;
+    Scratch<int32_t> sc;
+    ARBX_TRY(sq.alloc((size_t)nq * w, s));
+    ARBX_TRY(sc.alloc((size_t)nq, s));
+    gather_rows_kernel<<<(unsigned)((nq * w + 255) / 256), 256, 0, s>>>(queries, order.p, nq, w, sq.p);
+    ARBX_LAUNCH_CHECK();
+    a.queries = sq.p; a.qorder = nullptr; a.counts = sc.p;
+    ARBX_TRY(dim_table(ix->dim)->spatial(ix, a, s));
+    unpermute_i32_kernel<<<(unsigned)((nq + 255) / 256), 256, 0, s>>>(sc.p, order.p, nq, counts);
+    ARBX_LAUNCH_CHECK();
+    return ARBX_OK;
+  }
   return dim_table(ix->dim)->spatial(ix, a, s);
 }
 
@@ -740,6 +771,7 @@ arbx_status arbx_debug_set(const char* key, double value) {
   else if (k == "code_bits") g_cfg.code_bits.store(iv);
   else if (k == "brute_max") g_cfg.brute_max.store(iv);
   else if (k == "l2_persist") g_cfg.l2_persist.store(iv);
+  else if (k == "gather") g_cfg.gather.store(iv);
   else if (k == "packet_alpha") g_cfg.packet_alpha.store((float)value);
   else if (k == "pool_keep_mb") {
     g_pool_keep_mb.store((long long)value);
@@ -748,7 +780,7 @@ arbx_status arbx_debug_set(const char* key, double value) {
     if (cudaMemPool_t pool = pool_for(dev)) pool_apply_threshold(pool);
   } else if (k == "reset") {
     g_cfg.leaf_max.store(16); g_cfg.store_budget_mb.store(4096); g_cfg.traversal.store(0); g_cfg.qbits.store(0);
-    g_cfg.code_bits.store(0); g_cfg.brute_max.store(-1); g_cfg.l2_persist.store(0); g_cfg.packet_alpha.store(-1.f);
+    g_cfg.code_bits.store(0); g_cfg.brute_max.store(-1); g_cfg.gather.store(0); g_cfg.l2_persist.store(0); g_cfg.packet_alpha.store(-1.f);
   } else {
     set_error("arbx_debug_set: unknown key '%s'", key);
     return ARBX_ERR_INVALID_ARG;

@@ -64,6 +64,7 @@ struct DebugCfg {
   std::atomic<int> qbits{0};            // query-code bits per axis kept for the query sort (0 = all)
   std::atomic<int> code_bits{0};        // primitive-code bits per axis (0 = adapted to n)
   std::atomic<int> brute_max{-1};       // n <= brute_max builds a brute-force index (-1 = default)
+  std::atomic<int> gather{0};           // 1: arbx_query_count materialises the sorted queries (Q3 experiment)
   std::atomic<int> l2_persist{0};       // 1: persisting-L2 window over the node array during queries
   std::atomic<float> packet_alpha{-1.f};   // packet threshold (< 0 = default per kind / dim)
 };
