@@ -438,3 +438,16 @@ def test_f64_edges_and_type_checks(arbx):
     assert off0.cpu().tolist() == [0]
     for ix in (ix64, ix32, ix64t, e, small):
         ix.close()
+
+
+def test_gather_knob_does_not_change_results(arbx, knobs):
+    """The Q3 experiment (sorted copy of the queries + un-permuted counts) is only another route."""
+    p = _dev(dg.uniform_points(100_000, 3, 1))
+    q = _dev(dg.sphere_queries(dg.uniform_points(30_001, 3, 2), 0.03))
+    qb = _dev(dg.uniform_boxes(10_007, 3, 3, 0.02))
+    ix = arbx.Index(p, dg.POINT)
+    a, ab = ix.query_count(q), ix.query_count(qb, dg.BOX)
+    knobs(gather=1)
+    b, bb = ix.query_count(q), ix.query_count(qb, dg.BOX)
+    assert torch.equal(a, b) and torch.equal(ab, bb) and int(a.sum()) > 0
+    ix.close()
