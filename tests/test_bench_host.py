@@ -76,3 +76,16 @@ def test_max_over_ranks_gloo_world2(tmp_path):
         out, err = p.communicate(timeout=120)
         assert p.returncode == 0, err
         assert out.startswith("ok")
+
+
+def test_gpus_flag_starts_the_ranks_itself():
+    """`python bench.py --gpus 2` outside torchrun re-executes itself under torch.distributed.run
+    with 2 ranks (it used to run one rank and print n_gpus 1).  Checked on the
+    reference arm, which needs no GPU: rank 0 prints the line, rank 1 exits quietly."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference",
+                          "--workload", "C1", "--steps", "1", "--warmup", "0"], capture_output=True, text=True,
+                         cwd=ROOT, env=env, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(l) for l in out.stdout.strip().splitlines() if l.startswith("{")]
+    assert len(lines) == 1 and lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2
