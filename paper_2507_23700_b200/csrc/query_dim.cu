@@ -827,7 +827,8 @@ __global__ void __launch_bounds__(QT) knn_packet_kernel(const float4* __restrict
                                                         const int32_t* __restrict__ kq, int kmax,
                                                         int32_t* __restrict__ indices,
                                                         float* __restrict__ distances,
-                                                        uint8_t* __restrict__ fallback, float alpha, int force) {
+                                                        uint32_t* __restrict__ wlist, uint32_t* __restrict__ wcount,
+                                                        float alpha, int force) {
   using Heap = RegHeap<KB>;
   constexpr int PQ_CAP = 320;                       // node work list per warp
   constexpr int RCAP = 96;                          // candidate leaf ranges per warp (3 per lane)
@@ -917,7 +918,7 @@ __global__ void __launch_bounds__(QT) knn_packet_kernel(const float4* __restrict
     const float ub = __uint_as_float(prefix | 0x7fffu);
     const float dk = PK == KIND_SPHERE ? ub : sqrtf(ub);
     if (!force && !(dmax <= alpha * dk)) {   // not coherent: one query per lane does it
-      if (lane == 0) fallback[wfirst >> 5] = 1;
+      if (lane == 0) wlist[atomicAdd(wcount, 1u)] = (uint32_t)(wfirst >> 5);
       KSTAT(1, 1);
       return;
     }
@@ -972,7 +973,7 @@ __global__ void __launch_bounds__(QT) knn_packet_kernel(const float4* __restrict
       const uint32_t r0 = __ballot_sync(~0u, lf0), r1 = __ballot_sync(~0u, lf1);
       const int nr = __popc(r0) + __popc(r1);
       if (nranges + nr > RCAP) {               // more candidate ranges than the list holds: per-lane kernel
-        if (lane == 0) fallback[wfirst >> 5] = 1;
+        if (lane == 0) wlist[atomicAdd(wcount, 1u)] = (uint32_t)(wfirst >> 5);
         KSTAT(1, 1);
         return;
       }
@@ -1077,18 +1078,14 @@ __global__ void __launch_bounds__(QT) knn_packet_kernel(const float4* __restrict
 // (high dimension, strongly clustered data) the packet visits the union of 32 unrelated
 // paths and independent traversal wins.  Spatial kernels choose per warp (warp_coherent).
 template <int PK, class Heap>
-__global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict__ nodes,
+__device__ __forceinline__ void knn_thread_query(const int64_t t, const float4* __restrict__ nodes,
                                                  const float4* __restrict__ leaves,
                                                  const int32_t* __restrict__ root,
                                                  const float* __restrict__ qpoints,
-                                                 const uint32_t* __restrict__ qorder, int64_t nq,
+                                                 const uint32_t* __restrict__ qorder,
                                                  const int32_t* __restrict__ kq, int kmax,
                                                  int64_t n, int32_t* __restrict__ indices,
-                                                 float* __restrict__ distances,
-                                                 const uint8_t* __restrict__ only, int vec_ok) {
-  const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
-  if (t >= nq) return;
-  if (only && !only[t >> 5]) return;   // this warp was answered by the packet kernel
+                                                 float* __restrict__ distances, int vec_ok) {
   const int64_t qi = qorder ? (int64_t)qorder[t] : t;
   float y[D];
 #pragma unroll
@@ -1157,6 +1154,40 @@ __global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict
   }
 }
 
+template <int PK, class Heap>
+__global__ void __launch_bounds__(QT) knn_thread_kernel(const float4* __restrict__ nodes,
+                                                 const float4* __restrict__ leaves,
+                                                 const int32_t* __restrict__ root,
+                                                 const float* __restrict__ qpoints,
+                                                 const uint32_t* __restrict__ qorder, int64_t nq,
+                                                 const int32_t* __restrict__ kq, int kmax,
+                                                 int64_t n, int32_t* __restrict__ indices,
+                                                 float* __restrict__ distances, int vec_ok) {
+  const int64_t t = (int64_t)blockIdx.x * QT + threadIdx.x;
+  if (t < nq) knn_thread_query<PK, Heap>(t, nodes, leaves, root, qpoints, qorder, kq, kmax, n, indices, distances, vec_ok);
+}
+
+// The warps the packet kernel handed over (list `wlist` of warp numbers, `*wcount` entries): a
+// fixed grid walks the list, so every resident warp has work for the whole launch (a launch
+// over all warps with an early exit ran at 34 % active warps).
+template <int PK, class Heap>
+__global__ void __launch_bounds__(QT) knn_thread_list_kernel(const float4* __restrict__ nodes,
+                                                 const float4* __restrict__ leaves,
+                                                 const int32_t* __restrict__ root,
+                                                 const float* __restrict__ qpoints,
+                                                 const uint32_t* __restrict__ qorder, int64_t nq,
+                                                 const int32_t* __restrict__ kq, int kmax,
+                                                 int64_t n, int32_t* __restrict__ indices,
+                                                 float* __restrict__ distances, int vec_ok,
+                                                 const uint32_t* __restrict__ wlist,
+                                                 const uint32_t* __restrict__ wcount) {
+  const uint32_t cnt = *wcount;
+  for (uint32_t i = blockIdx.x * (QT / 32) + (threadIdx.x >> 5); i < cnt; i += gridDim.x * (QT / 32)) {
+    const int64_t t = (int64_t)wlist[i] * 32 + (threadIdx.x & 31);
+    if (t < nq) knn_thread_query<PK, Heap>(t, nodes, leaves, root, qpoints, qorder, kq, kmax, n, indices, distances, vec_ok);
+  }
+}
+
 inline int traversal_mode() { return g_cfg.traversal.load(std::memory_order_relaxed); }
 
 // ---- host dispatch ------------------------------------------------------------------------------------
@@ -1207,18 +1238,27 @@ arbx_status spatial_entry(const Index* ix, const SpatialArgs& a, cudaStream_t s)
 }
 
 template <int PK, class Heap>
-arbx_status knn_thread_launch(const Index* ix, const KnnArgs& a, const uint8_t* only, cudaStream_t s) {
-  const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);
+arbx_status knn_thread_launch(const Index* ix, const KnnArgs& a, const uint32_t* wlist, const uint32_t* wcount, cudaStream_t s) {
   // 128-bit row stores need 16-byte aligned output pointers (rows of 4, 8, 16, 32 entries then stay aligned)
   const int vec_ok = !a.kq && ((reinterpret_cast<uintptr_t>(a.indices) | reinterpret_cast<uintptr_t>(a.distances)) & 15) == 0;
-  knn_thread_kernel<PK, Heap><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
-                                                  reinterpret_cast<const float4*>(ix->leaves), ix->root, a.qpoints,
-                                                  a.qorder, a.nq, a.kq, a.k, ix->n, a.indices, a.distances, only, vec_ok);
+  const float4* nodes = reinterpret_cast<const float4*>(ix->nodes);
+  const float4* leaves = reinterpret_cast<const float4*>(ix->leaves);
+  if (wlist) {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    knn_thread_list_kernel<PK, Heap><<<sms * 16, QT, 0, s>>>(nodes, leaves, ix->root, a.qpoints, a.qorder, a.nq, a.kq, a.k, ix->n,
+                                                            a.indices, a.distances, vec_ok, wlist, wcount);
+  } else {
+    const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);
+    knn_thread_kernel<PK, Heap><<<grid, QT, 0, s>>>(nodes, leaves, ix->root, a.qpoints, a.qorder, a.nq, a.kq, a.k, ix->n,
+                                                    a.indices, a.distances, vec_ok);
+  }
   ARBX_LAUNCH_CHECK();
   return ARBX_OK;
 }
 
-// Packet kernel for the coherent warps, per-lane kernel for the rest (flagged per warp).
+// Packet kernel for the coherent warps, per-lane kernel for the rest (listed by the packet kernel).
 template <int PK, int KB>
 arbx_status knn_launch(const Index* ix, const KnnArgs& a, cudaStream_t s) {
   ProfScope ps(K_KNN, s);
@@ -1228,24 +1268,24 @@ arbx_status knn_launch(const Index* ix, const KnnArgs& a, cudaStream_t s) {
   //  longer one: C1, 10^4 queries, 0.20 ms with packets against 0.14 ms without)
   const bool packet = mode != 1 && ix->n >= 4 * (int64_t)a.k && ix->n > 4 * (int64_t)ix->leaf_max && ix->n >= 64 &&
                       (a.nq >= 65536 || mode == 2);
-  if (!packet) return knn_thread_launch<PK, RegHeap<KB>>(ix, a, nullptr, s);
-  const int64_t nwarps = (a.nq + 31) / 32;
-  Scratch<uint8_t> flags;
-  ARBX_TRY(flags.alloc((size_t)nwarps, s));
-  ARBX_CUDA(cudaMemsetAsync(flags.p, 0, (size_t)nwarps, s));
+  if (!packet) return knn_thread_launch<PK, RegHeap<KB>>(ix, a, nullptr, nullptr, s);
   // measured: above 3-D the warps of the clustered workload (C5) are never coherent and the seed
   // descent is pure overhead (+0.7 ms per 10^7 queries), so packets are off unless asked for
   float alpha = D <= 3 ? 2.0f : 0.f;
   if (const float v = g_cfg.packet_alpha.load(std::memory_order_relaxed); v >= 0.f) alpha = v;
-  if (alpha <= 0.f && mode != 2) return knn_thread_launch<PK, RegHeap<KB>>(ix, a, nullptr, s);
+  if (alpha <= 0.f && mode != 2) return knn_thread_launch<PK, RegHeap<KB>>(ix, a, nullptr, nullptr, s);
+  const int64_t nwarps = (a.nq + 31) / 32;
+  Scratch<uint32_t> wlist;   // [0] = number of listed warps, [1 ..] = their numbers
+  ARBX_TRY(wlist.alloc((size_t)nwarps + 1, s));
+  ARBX_CUDA(cudaMemsetAsync(wlist.p, 0, sizeof(uint32_t), s));
   const unsigned grid = (unsigned)((a.nq + QT - 1) / QT);
   knn_packet_kernel<PK, KB><<<grid, QT, 0, s>>>(reinterpret_cast<const float4*>(ix->nodes),
                                                 reinterpret_cast<const float4*>(ix->leaves), ix->root, (int)ix->n,
                                                 a.qpoints, a.qorder, a.nq, a.kq, a.k, a.indices, a.distances,
-                                                flags.p, alpha, mode == 2 ? 1 : 0);
+                                                wlist.p + 1, wlist.p, alpha, mode == 2 ? 1 : 0);
   ARBX_LAUNCH_CHECK();
   // (forced packets still leave the warps with too many candidate ranges to the per-lane kernel)
-  return knn_thread_launch<PK, RegHeap<KB>>(ix, a, flags.p, s);
+  return knn_thread_launch<PK, RegHeap<KB>>(ix, a, wlist.p + 1, wlist.p, s);
 }
 
 template <int PK>
@@ -1258,7 +1298,7 @@ arbx_status knn_pk(const Index* ix, const KnnArgs& a, cudaStream_t s) {
   if (k <= 16) return knn_launch<PK, 16>(ix, a, s);
   if (k <= 32) return knn_launch<PK, 32>(ix, a, s);
   ProfScope ps(K_KNN, s);
-  return knn_thread_launch<PK, LocalHeap>(ix, a, nullptr, s);
+  return knn_thread_launch<PK, LocalHeap>(ix, a, nullptr, nullptr, s);
 }
 
 arbx_status knn_entry(const Index* ix, const KnnArgs& a, cudaStream_t s) {
