@@ -127,9 +127,11 @@ _NCU_KERNEL = {"K1K2_knn": "knn_", "T1_spatial_count": "spatial_kernel", "T3_spa
                "Q2_qsort_pass": "onesweep_pass<unsigned int"}
 
 
-def ncu_traffic(kernel_id: str, workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-    committed ncu capture of this same workload (profiles/r2_launches_<workload>.csv); None if absent."""
+def ncu_traffic(kernel_id: str, workload: str, launches_per_step: float = 1.0):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel id per bracketed launch,
+    from the committed ncu launch list of this same workload (profiles/r2_launches_<workload>.csv
+    holds the rows of ONE step): the sum over every CUDA kernel of that id (K1K2_knn = packet +
+    per-lane kernel) divided by the number of bracketed launches per step; None if absent."""
     path = os.path.join(ROOT, "profiles", f"r2_launches_{workload}.csv")
     pat = _NCU_KERNEL.get(kernel_id)
     if not pat or not os.path.exists(path):
@@ -141,7 +143,7 @@ def ncu_traffic(kernel_id: str, workload: str):
             if pat in r["kernel"]:
                 tot += float(r["dram_read_bytes"]) + float(r["dram_write_bytes"])
                 cnt += 1
-    return int(tot / cnt) if cnt else None
+    return int(tot / max(launches_per_step, 1.0)) if cnt else None
 
 
 def max_over_ranks(vals, device=None):
@@ -690,7 +692,7 @@ def main():
         # per-LAUNCH figures for the dominant kernel
         lps = max(dk["launches_per_step"], 1)
         roofline = dict(bound="hbm", kernel=dom, achieved=dk["achieved_gbs"], peak=peak, unit="GB/s",
-                        frac=dk["frac_of_peak"], traffic=ncu_traffic(dom, cfg["name"]), peak_source=peak_src,
+                        frac=dk["frac_of_peak"], traffic=ncu_traffic(dom, cfg["name"], lps), peak_source=peak_src,
                         algorithmic_bytes_per_launch=int(ab[dom] / lps) if ab.get(dom) else None,
                         ms_per_launch=round(dk["ms_per_step"] / lps, 4), share_of_step=dk["share"])
         build_bytes = sum(ab[x] for x in ab if x.startswith("B"))
