@@ -187,6 +187,21 @@ ARBX_API arbx_status arbx_query_spatial_f64(arbx_handle h, const double* queries
 ARBX_API arbx_status arbx_query_knn_f64(arbx_handle h, const double* qpoints, int64_t nq, int k,
                                int32_t* indices, double* distances, arbx_stream stream);
 
+/* arbx_query_count for callers that must not allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same count-only search, same arguments,
+ * same results, but it calls no cudaMalloc / cudaFree / pool routine.  Its scratch (query codes,
+ * the sorted order, the sort's bookkeeping: 17.8 MB) is ONE fixed array inside the library, held by
+ * every GPU that loads the library until the process exits.  Limits and rules:
+ *   - nq <= ARBX_NOALLOC_MAX_QUERIES, otherwise ARBX_ERR_UNSUPPORTED (split the batch or use
+ *     arbx_query_count); fp32 handles only;
+ *   - every call on a device shares that one array: calls that overlap on the GPU (different
+ *     streams, or the same handle from two threads) RACE -- order them on one stream or with events;
+ *   - the array keeps the last call's contents; the call clears what it needs on `stream`.
+ * Asynchronous on `stream`.                                                                    */
+#define ARBX_NOALLOC_MAX_QUERIES (1 << 20)
+ARBX_API arbx_status arbx_query_count_noalloc(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                                     int32_t* counts, arbx_stream stream);
+
 /* Return the library's cached device memory on the current device to the driver, keeping at
  * most keep_bytes (0 = everything not in use).  Does not touch live handles.                 */
 ARBX_API arbx_status arbx_trim(int64_t keep_bytes);

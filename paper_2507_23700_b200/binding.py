@@ -26,6 +26,7 @@ EXPORTS = (
     "arbx_query_count_upto", "arbx_query_spatial", "arbx_query_spatial_upto", "arbx_query_pairs", "arbx_dbscan", "arbx_query_knn", "arbx_sort_pairs", "arbx_debug_validate",
     "arbx_query_knn_var", "arbx_trim", "arbx_debug_set",
     "arbx_build_f64", "arbx_query_count_f64", "arbx_query_spatial_f64", "arbx_query_knn_f64",
+    "arbx_query_count_noalloc",
     "arbx_launch_count", "arbx_profile_enable", "arbx_profile_num_kernels",
     "arbx_profile_kernel_name", "arbx_profile_read", "arbx_status_string", "arbx_last_error",
 )
@@ -67,6 +68,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_query_count_f64.argtypes = [vp, vp, i64, i32, vp, vp]
         L.arbx_query_spatial_f64.argtypes = [vp, vp, i64, i32, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.arbx_query_knn_f64.argtypes = [vp, vp, i64, i32, vp, vp, vp]
+        L.arbx_query_count_noalloc.argtypes = [vp, vp, i64, i32, vp, vp]
         L.arbx_trim.argtypes = [i64]
         L.arbx_debug_set.argtypes = [ctypes.c_char_p, ctypes.c_double]
         L.arbx_sort_pairs.argtypes = [vp, vp, i64, i32, i32, vp]
@@ -82,7 +84,7 @@ def lib() -> ctypes.CDLL:
         L.arbx_status_string.restype = ctypes.c_char_p
         L.arbx_status_string.argtypes = [i32]
         L.arbx_last_error.restype = ctypes.c_char_p
-        for name in EXPORTS[:20]:
+        for name in EXPORTS[:21]:
             getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -175,6 +177,16 @@ def arbx_query_count(handle: int, queries: torch.Tensor, nq: int, qkind: int, co
                      stream=None) -> None:
     _check(lib().arbx_query_count(handle, _ptr(queries), nq, qkind, _ptr(counts), _stream(stream)),
            "arbx_query_count")
+
+
+NOALLOC_MAX_QUERIES = 1 << 20
+
+
+def arbx_query_count_noalloc(handle: int, queries: torch.Tensor, nq: int, qkind: int, counts: torch.Tensor,
+                             stream=None) -> None:
+    """arbx_query_count without any allocation (fixed scratch inside the library, nq <= 2^20)."""
+    _check(lib().arbx_query_count_noalloc(handle, _ptr(queries), nq, qkind, _ptr(counts), _stream(stream)),
+           "arbx_query_count_noalloc")
 
 
 def arbx_query_count_upto(handle: int, queries: torch.Tensor, nq: int, qkind: int, limit: int,

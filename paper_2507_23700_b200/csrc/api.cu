@@ -730,6 +730,73 @@ arbx_status arbx_query_knn_f64(arbx_handle h, const double* qpoints, int64_t nq,
   return f64_knn(&h->ix, qpoints, order.p, nq, k, indices, distances, s);
 }
 
+// ---- arbx_query_count_noalloc: the count-only query without any allocation -------------------------
+// Its scratch (query codes and positions, both ping-pong halves, and the sort's meta words) lives in
+// ONE file-scope device array: every GPU that loads the library holds these 17.8 MB until exit.
+// In host code the array's name is only a stand-in, not a device address: the address is fetched
+// once per device, with that device current, by cudaGetSymbolAddress, and that pointer is what the
+// kernels get.
+constexpr int64_t kNoAllocMaxQueries = ARBX_NOALLOC_MAX_QUERIES;
+constexpr size_t kNoAllocMetaWords = 4 * 256 + 8 + 4 * (size_t)((kNoAllocMaxQueries + 4095) / 4096) * 256;   // 4 passes of 8 bits
+constexpr size_t kNoAllocWords = 4 * (size_t)kNoAllocMaxQueries + kNoAllocMetaWords;
+static __device__ __align__(256) uint32_t g_noalloc_scratch[kNoAllocWords];
+
+static std::once_flag g_noalloc_once[64];
+static uint32_t* g_noalloc_ptr[64];
+static cudaError_t g_noalloc_err[64];
+
+static arbx_status noalloc_scratch(uint32_t** out) {
+  int dev = 0;
+  ARBX_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) { set_error("arbx_query_count_noalloc: device %d out of range", dev); return ARBX_ERR_UNSUPPORTED; }
+  std::call_once(g_noalloc_once[dev], [dev] {   // the calling thread has `dev` current
+    void* p = nullptr;
+    g_noalloc_err[dev] = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    g_noalloc_ptr[dev] = g_noalloc_err[dev] == cudaSuccess ? static_cast<uint32_t*>(p) : nullptr;
+  });
+  if (!g_noalloc_ptr[dev]) {
+    set_error("arbx_query_count_noalloc: cudaGetSymbolAddress failed: %s", cudaGetErrorString(g_noalloc_err[dev]));
+    return ARBX_ERR_CUDA;
+  }
+  *out = g_noalloc_ptr[dev];
+  return ARBX_OK;
+}
+
+arbx_status arbx_query_count_noalloc(arbx_handle h, const float* queries, int64_t nq, arbx_kind qkind,
+                                     int32_t* counts, arbx_stream stream) {
+  if (!h || nq < 0 || bad_kind((int)qkind) || (nq > 0 && (!queries || !counts))) {
+    set_error("arbx_query_count_noalloc: invalid argument");
+    return ARBX_ERR_INVALID_ARG;
+  }
+  if (h->ix.f64) { set_error("arbx_query_count_noalloc: fp32 handles only"); return ARBX_ERR_INVALID_ARG; }
+  if (nq > kNoAllocMaxQueries) {
+    set_error("arbx_query_count_noalloc: nq = %lld exceeds ARBX_NOALLOC_MAX_QUERIES = %lld (the fixed scratch array); "
+              "use arbx_query_count or split the batch", (long long)nq, (long long)kNoAllocMaxQueries);
+    return ARBX_ERR_UNSUPPORTED;
+  }
+  if (nq == 0) return ARBX_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  const Index* ix = &h->ix;
+  if (ix->n == 0) { ARBX_CUDA(cudaMemsetAsync(counts, 0, (size_t)nq * sizeof(int32_t), s)); return ARBX_OK; }
+  const uint32_t* order = nullptr;
+  if (!ix->brute) {   // Q1 + Q2 in the static scratch (a brute-force index scans everything: no order needed)
+    uint32_t* base = nullptr;
+    ARBX_TRY(noalloc_scratch(&base));
+    uint32_t* codes = base;
+    uint32_t* codes_alt = base + kNoAllocMaxQueries;
+    uint32_t* ord0 = base + 2 * kNoAllocMaxQueries;
+    uint32_t* ord1 = base + 3 * kNoAllocMaxQueries;
+    uint32_t* meta = base + 4 * kNoAllocMaxQueries;
+    int key_bits = 32;
+    ARBX_TRY(dim_table(ix->dim)->qcode(ix, queries, nq, (int)qkind, codes, &key_bits, s));
+    uint32_t *kout = nullptr, *vout = nullptr;
+    ARBX_TRY(radix_sort_u32_noalloc(codes, codes_alt, ord0, ord1, nq, key_bits, meta, kNoAllocMetaWords, s, &kout, &vout));
+    order = vout;
+  }
+  SpatialArgs a{queries, nq, (int)qkind, order, counts, nullptr, nullptr, nullptr, 0, nullptr, 0};
+  return dim_table(ix->dim)->spatial(ix, a, s);
+}
+
 arbx_status arbx_sort_pairs(void* keys, uint32_t* values, int64_t n, int key_bytes, int key_bits,
                             arbx_stream stream) {
   if (n < 0 || (n > 0 && !keys) || (key_bytes != 4 && key_bytes != 8) || key_bits < 1 || key_bits > 8 * key_bytes) {

@@ -142,6 +142,12 @@ arbx_status radix_sort_u32(uint32_t* keys, uint32_t* keys_alt, uint32_t* vals, u
                            bool iota_vals, int64_t n, int key_bits, cudaStream_t s,
                            uint32_t** keys_out, uint32_t** vals_out);
 
+// sort.cu: the 32-bit query sort (values = positions) on caller-provided buffers only, `meta` included
+size_t sort_meta_words(int64_t n, int key_bits);
+arbx_status radix_sort_u32_noalloc(uint32_t* keys, uint32_t* keys_alt, uint32_t* vals, uint32_t* vals_alt, int64_t n,
+                                   int key_bits, uint32_t* meta, size_t meta_capacity_words, cudaStream_t s,
+                                   uint32_t** keys_out, uint32_t** vals_out);
+
 // build.cu
 arbx_status build_index(const float* prims, int64_t n, int dim, int kind, cudaStream_t s,
                         Index* ix);

@@ -8,6 +8,7 @@
 //
 // Algorithmic HBM bytes per element: histogram K; per pass 2*(K+4)
 // (K = key bytes; the first pass of an iota sort reads no values).
+#include <algorithm>
 #include <atomic>
 
 #include "common.cuh"
@@ -371,6 +372,69 @@ arbx_status radix_sort_impl(K* keys, K* kalt, uint32_t* vals, uint32_t* valt, bo
 }
 
 }  // namespace
+
+// The query sort (32-bit keys, values = positions) with every buffer provided by the caller,
+// including the sort's own `meta` words (digit histograms, tile tickets, look-back status:
+// sort_meta_words(n, key_bits) of them, cleared here on the stream).  Calls no allocator: this
+// is the sort of arbx_query_count_noalloc.  Same kernels as radix_sort_u32.
+size_t sort_meta_words(int64_t n, int key_bits) {
+  const int npass = (std::max(key_bits, 1) + 7) / 8;
+  const size_t ntiles = (size_t)((n + SORT_TILE - 1) / SORT_TILE);
+  return (size_t)npass * 256 + MAX_PASSES + (size_t)npass * ntiles * 256;
+}
+arbx_status radix_sort_u32_noalloc(uint32_t* keys, uint32_t* kalt, uint32_t* vals, uint32_t* valt, int64_t n,
+                                   int key_bits, uint32_t* meta, size_t meta_capacity_words, cudaStream_t s,
+                                   uint32_t** keys_out, uint32_t** vals_out) {
+  using K = uint32_t;
+  constexpr int BITS = 8, RADIX = 256;
+  *keys_out = keys;
+  *vals_out = vals;
+  if (n <= 0) return ARBX_OK;
+  if (n == 1) { ARBX_CUDA(cudaMemsetAsync(vals, 0, sizeof(uint32_t), s)); return ARBX_OK; }
+  key_bits = std::max(1, std::min(32, key_bits));
+  const int npass = (key_bits + BITS - 1) / BITS;
+  const uint32_t top_mask = key_bits % BITS ? (1u << (key_bits % BITS)) - 1u : (uint32_t)(RADIX - 1);
+  const uint32_t ntiles = (uint32_t)((n + SORT_TILE - 1) / SORT_TILE);
+  const size_t meta_words = sort_meta_words(n, key_bits);
+  if (meta_words > meta_capacity_words) { set_error("radix sort (no-alloc): meta buffer too small"); return ARBX_ERR_UNSUPPORTED; }
+  ARBX_CUDA(cudaMemsetAsync(meta, 0, meta_words * sizeof(uint32_t), s));   // the buffer keeps the last call's contents
+  uint32_t* ghist = meta;
+  uint32_t* counters = meta + (size_t)npass * RADIX;
+  uint32_t* status = counters + MAX_PASSES;
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  {
+    ProfScope ps(K_QSORT_HIST, s);
+    const int64_t want = (n / 4 + 511) / 512;
+    const int grid = (int)std::min<int64_t>(std::max<int64_t>(want, 1), (int64_t)sms * 4);
+    hist_kernel<K, BITS><<<grid, 512, 0, s>>>(keys, (uint32_t)n, npass, top_mask, ghist);
+    ARBX_LAUNCH_CHECK();
+    hist_scan_kernel<BITS><<<npass, 256, 0, s>>>(ghist);
+    ARBX_LAUNCH_CHECK();
+  }
+  const size_t smem_kv = sizeof(K) * SORT_TILE + sizeof(uint32_t) * SORT_WARPS * (RADIX / 2) + sizeof(uint32_t) * SORT_TILE;
+  ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, BITS, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_kv));
+  ARBX_CUDA(cudaFuncSetAttribute(onesweep_pass<K, BITS, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_kv));
+  K* kin = keys; K* kout = kalt;
+  uint32_t* vin = vals; uint32_t* vout = valt;
+  for (int p = 0; p < npass; ++p) {
+    const uint32_t* base = ghist + (size_t)p * RADIX;
+    uint32_t* st = status + (size_t)p * ntiles * RADIX;
+    const uint32_t dmask = p == npass - 1 ? top_mask : (uint32_t)(RADIX - 1);
+    ProfScope ps(K_QSORT_PASS, s);
+    if (p == 0)
+      onesweep_pass<K, BITS, true, true><<<ntiles, SORT_THREADS, smem_kv, s>>>(kin, kout, nullptr, vout, (uint32_t)n, BITS * p, dmask, base, counters + p, st);
+    else
+      onesweep_pass<K, BITS, false, true><<<ntiles, SORT_THREADS, smem_kv, s>>>(kin, kout, vin, vout, (uint32_t)n, BITS * p, dmask, base, counters + p, st);
+    ARBX_LAUNCH_CHECK();
+    std::swap(kin, kout);
+    std::swap(vin, vout);
+  }
+  *keys_out = kin;
+  *vals_out = vin;
+  return ARBX_OK;
+}
 
 arbx_status radix_sort_u64(unsigned long long* keys, unsigned long long* keys_alt, uint32_t* vals,
                            uint32_t* vals_alt, bool iota_vals, int64_t n, int key_bits,
