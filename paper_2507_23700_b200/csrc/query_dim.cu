@@ -1004,11 +1004,14 @@ __global__ void __launch_bounds__(QT) knn_packet_kernel(const float4* __restrict
 #pragma unroll
       for (int j = 1; j < RCAP / 32; ++j)
         if (rd[j] < best) { best = rd[j]; bi = j * 32 + lane; }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        const float ob = __shfl_xor_sync(~0u, best, o);
-        const int oi = __shfl_xor_sync(~0u, bi, o);
-        if (ob < best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+      // warp argmin with redux.sync: box distances are >= 0 (or +inf), so their bit patterns
+      // order like the values; among equal minima the lowest lane's range is taken
+      {
+        const uint32_t bb = __float_as_uint(best);
+        const uint32_t mb = __reduce_min_sync(~0u, bb);
+        const int src = __ffs(__ballot_sync(~0u, bb == mb)) - 1;
+        bi = __shfl_sync(~0u, bi, src);
+        best = __uint_as_float(mb);
       }
       if (!(best < rj)) break;
 #pragma unroll
@@ -1040,9 +1043,7 @@ __global__ void __launch_bounds__(QT) knn_packet_kernel(const float4* __restrict
           }
         }
       }
-      rj = thr;
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) rj = fmaxf(rj, __shfl_xor_sync(~0u, rj, o));
+      rj = __uint_as_float(__reduce_max_sync(~0u, __float_as_uint(thr)));   // thr >= 0: bits order like values
     }
   }
 
